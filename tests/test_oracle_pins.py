@@ -1,0 +1,383 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these re-types the oracle's formulas: they use known-answer vectors, closed forms,
+invariants, a brute-force quadrature and explicit python bond loops.  CPU only.
+"""
+import os
+
+import numpy as np
+import pytest
+from scipy.special import i0, i1
+
+from paper_1211_0780_b200 import inputs
+from tests import helpers as H
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+SEED = inputs.SEED
+
+
+def _kat_rows():
+    rows = []
+    with open(os.path.join(GOLDEN, "philox4x32_10_kat.txt")) as f:
+        for line in f:
+            line = line.strip()
+            if not line or line.startswith("#"):
+                continue
+            w = [int(t, 16) for t in line.split()]
+            rows.append((w[0:4], w[4:6], w[6:10]))
+    assert len(rows) == 3
+    return rows
+
+
+# ------------------------------------------------------------------------------ RNG -----
+def test_philox_known_answers(oracle_mod):
+    for ctr, key, want in _kat_rows():
+        got = oracle_mod.philox4x32_10(ctr, key)
+        assert [int(x) for x in got] == want
+
+
+def test_helper_philox_known_answers_and_agreement(oracle_mod):
+    # the test-side numpy Philox (used to predict draws) is pinned by the same vectors ...
+    for ctr, key, want in _kat_rows():
+        got = H.philox4x32_10_np(*ctr, *key)
+        assert [int(x) for x in got] == want
+    # ... and agrees with the oracle's on random counters/keys
+    rng = np.random.default_rng(1)
+    for _ in range(200):
+        ctr = rng.integers(0, 2 ** 32, 4, dtype=np.uint64)
+        key = rng.integers(0, 2 ** 32, 2, dtype=np.uint64)
+        a = oracle_mod.philox4x32_10(ctr, key)
+        b = H.philox4x32_10_np(*ctr, *key)
+        assert [int(x) for x in a] == [int(x) for x in b]
+
+
+def test_u24_moments():
+    W = H.philox4x32_10_np(np.arange(250000), 3, 5, 1, 123, 456)
+    u = np.concatenate([H.u24(w) for w in W]).astype(np.float64)
+    assert u.min() >= 0.0 and u.max() < 1.0
+    n = u.size
+    assert abs(u.mean() - 0.5) < 5 / np.sqrt(12 * n)
+    assert abs(u.var() - 1 / 12) < 5 * np.sqrt(1 / 180 / n)
+    hist, _ = np.histogram(u, bins=256, range=(0, 1))
+    chi2 = ((hist - n / 256) ** 2 / (n / 256)).sum()
+    assert chi2 < 255 + 6 * np.sqrt(2 * 255)
+
+
+# ------------------------------------------------------------------ init + O1 (beta=0) --
+def test_init_random_is_predictable_from_philox_alone(oracle_mod):
+    L, R = 8, 3
+    o = oracle_mod.XYOracle(L, R, [0.4, 0.5, 0.6], SEED)
+    o.init_random()
+    want = H.predicted_init(L, R, SEED)
+    got = o.get_state()
+    assert np.array_equal(got.view(np.uint32), want.view(np.uint32))
+    assert got.min() >= 0 and got.max() < 2 * np.pi + 1e-6
+
+
+@pytest.mark.parametrize("L,n_met", [(4, 0), (8, 7), (6, 3)])
+def test_O1_beta0_accepts_every_proposal_bit_exactly(oracle_mod, L, n_met):
+    R = 2
+    o = oracle_mod.XYOracle(L, R, [0.0, 0.0], SEED)
+    o.set_state(inputs.uniform_state(L, R, 5))
+    o.set_counters([n_met, 0, 0])
+    o.metropolis_sweep()
+    prop, _ = H.predicted_proposals(L, R, n_met, SEED)
+    got = o.get_state()
+    assert np.array_equal(got.view(np.uint32), prop.view(np.uint32))
+    assert o.get_counters()[0] == n_met + 1
+    met, _ = o.get_accept_counts()
+    assert np.all(met == L ** 3)
+    # black and white neighbours must not share random numbers (reading R12)
+    assert np.all(got != np.roll(got, 1, axis=3))
+
+
+def test_O1_beta0_energy_moments(oracle_mod):
+    L, R, T = 4, 64, 150
+    o = oracle_mod.XYOracle(L, R, np.zeros(R), SEED)
+    o.init_random()
+    E = np.empty((T, R))
+    for t in range(T):
+        o.metropolis_sweep()
+        E[t] = o.measure()[:, 0]
+    N = L ** 3
+    n = E.size
+    assert abs(E.mean()) < 5 * np.sqrt(1.5 * N / n)           # <E> = 0
+    assert abs(E.var() / (1.5 * N) - 1) < 0.06                # var(E) = 3N/2 (3N bonds, var(cos)=1/2)
+
+
+# ----------------------------------------------------------------- O2 high-T series -----
+def test_O2_high_temperature_series(oracle_mod):
+    """<cos> per bond = t + 8 t^3 t' + O(t^5), t = I1/I0, t' = dt/dbeta: tree level plus the four
+    plaquettes through a bond (from ln Z = 3N ln I0 + 3N * 2 t^4 + ...)."""
+    beta, L, R, T, burn = 0.1, 8, 32, 700, 20
+    t = i1(beta) / i0(beta)
+    tp = 1 - t / beta - t * t
+    want = -3 * (t + 8 * t ** 3 * tp)
+    assert abs(want - (-0.15130)) < 2e-5                       # the value SURVEY.md quotes
+    o = oracle_mod.XYOracle(L, R, np.full(R, beta), SEED, threads=4)
+    o.init_random()
+    E = np.empty((T, R))
+    for k in range(burn + T):
+        o.metropolis_sweep()
+        if k >= burn:
+            E[k - burn] = o.measure()[:, 0]
+    mean, err = H.mean_and_err_over_replicas(E / L ** 3)
+    assert err < 6e-4
+    assert abs(mean - want) < 4 * err + 2e-4, (mean, want, err)
+    assert abs(mean - (-3 * t)) > 1.5 * err                    # and it does resolve beyond tree level
+
+
+# ------------------------------------------------------------------- O3 T=0 fixed point --
+def test_O3_zero_temperature_fixed_point(oracle_mod):
+    L, R = 6, 2
+    o = oracle_mod.XYOracle(L, R, [1e30, 1e30], SEED)
+    o.init_ordered(0.0)
+    for _ in range(3):
+        o.metropolis_sweep()
+        o.overrelax_sweep()
+    s = o.get_state()
+    assert np.all(s == 0.0)
+    N = L ** 3
+    obs = o.measure()
+    assert np.allclose(obs[:, 0], -3 * N, rtol=0, atol=1e-9)
+    assert np.allclose(obs[:, 1], N) and np.allclose(obs[:, 2], 0)
+    assert np.allclose(obs[:, 3], N ** 2) and np.allclose(obs[:, 4], float(N) ** 4)
+    assert np.all(o.get_accept_counts()[0] <= 3 * 2)           # only theta'=0 exactly could be "accepted"
+
+
+# ---------------------------------------------------------------- O4/O5 over-relaxation --
+def test_O4_overrelaxation_conserves_energy(oracle_mod):
+    L, R = 8, 4
+    o = oracle_mod.XYOracle(L, R, [0.3, 0.45, 0.6, 1.0], SEED)
+    o.init_random()
+    for _ in range(3):
+        o.metropolis_sweep()
+    for _ in range(4):
+        E0 = o.measure()[:, 0]
+        before = o.get_state()
+        o.overrelax_sweep()
+        E1 = o.measure()[:, 0]
+        assert np.all(np.abs(E1 - E0) <= 1e-5 * np.abs(E0))   # north_star bound
+        assert np.all(np.abs(E1 - E0) <= 2e-7 * np.abs(E0))   # what fp32 storage actually leaves
+        assert np.mean(H.angle_diff(before, o.get_state()) > 1e-3) > 0.9   # and it does move spins
+
+
+def test_O5_overrelaxation_pass_is_an_involution(oracle_mod):
+    L, R = 8, 2
+    o = oracle_mod.XYOracle(L, R, [0.45, 0.45], SEED)
+    s0 = inputs.uniform_state(L, R, 11)
+    for colour in (0, 1):
+        o.set_state(s0)
+        tr = o.enable_trace(overrelax=True)
+        o.overrelax_pass(colour)
+        s1 = o.get_state()
+        h = tr["or_h"].copy()
+        o.overrelax_pass(colour)
+        s2 = o.get_state()
+        mask = np.broadcast_to(H.colour_mask(L)[None] == colour, s0.shape)
+        assert np.array_equal(s1[~mask], s0[~mask])            # the other colour is untouched
+        d = H.angle_diff(s2, s0)
+        hh = np.where(mask, h, 1.0)
+        assert np.all(d <= 2e-6 / np.minimum(hh, 1.0) + 1e-6)  # theta -> 2phi-theta twice, up to fp32 storage
+        assert np.mean(H.angle_diff(s1, s0)[mask] > 1e-3) > 0.9
+
+
+# ------------------------------------------------------------------------- measure pins --
+def test_measure_matches_brute_force_bond_loop(oracle_mod):
+    L, R = 4, 3
+    s = inputs.uniform_state(L, R, 21)
+    o = oracle_mod.XYOracle(L, R, [0.4, 0.5, 0.6], SEED)
+    o.set_state(s)
+    obs = o.measure()
+    for r in range(R):
+        want = H.brute_force_observables(s[r])
+        assert np.allclose(obs[r], want, rtol=1e-12, atol=1e-10)
+
+
+def test_O6_rotation_invariance(oracle_mod):
+    L, R = 8, 1
+    o = oracle_mod.XYOracle(L, R, [0.45], SEED)
+    s = inputs.uniform_state(L, R, 4).astype(np.float64)
+    o.set_state(s.astype(np.float32))
+    base = o.measure()[0]
+    for c in (0.5, 2.0, 4.0):
+        # the rotated state has to be representable: rotate in double, round to fp32, and compare
+        # with the brute-force value of THAT fp32 state -- the invariance itself is tested on E.
+        rot = ((s + c) % (2 * np.pi)).astype(np.float32)
+        o.set_state(rot)
+        obs = o.measure()[0]
+        assert abs(obs[0] - base[0]) < 3e-6 * abs(base[0]) + 1e-3          # fp32 rounding of the angles
+        assert abs(obs[3] - base[3]) < 1e-4 * max(base[3], 1.0) + 1.0      # |M|^2 is rotation invariant
+
+
+@pytest.mark.parametrize("k", [(1, 0, 0), (0, 1, 0), (0, 0, 1), (2, 1, 3), (0, 3, 0)])
+def test_O7_helical_state(oracle_mod, k):
+    L, R = 8, 1
+    o = oracle_mod.XYOracle(L, R, [0.45], SEED)
+    s = inputs.helical_state(L, R, k, phase=0.3)
+    o.set_state(s)
+    N = L ** 3
+    obs = o.measure()[0]
+    want = -N * sum(np.cos(2 * np.pi * kk / L) for kk in k)
+    assert abs(obs[0] - want) < 2e-6 * 3 * N
+    assert abs(obs[1]) < 1e-4 * N and abs(obs[2]) < 1e-4 * N
+    # h_i is parallel to S_i (or vanishes), so the state is a fixed point of over-relaxation
+    o.overrelax_sweep()
+    h_zero = abs(sum(np.cos(2 * np.pi * kk / L) for kk in k)) < 1e-9
+    if not h_zero:
+        assert np.max(H.angle_diff(o.get_state(), s)) < 5e-6
+
+
+def test_O8_staggered_state(oracle_mod):
+    L, R = 6, 1
+    o = oracle_mod.XYOracle(L, R, [0.45], SEED)
+    o.set_state(inputs.staggered_state(L, R))
+    obs = o.measure()[0]
+    N = L ** 3
+    assert abs(obs[0] - 3 * N) < 1e-5 * N
+    assert abs(obs[1]) < 1e-5 * N and abs(obs[2]) < 1e-5 * N
+
+
+# ------------------------------------------------------------------------ O9 L=2 exact --
+def test_exact_L2_quadrature_converged():
+    # spectral convergence: M=6 -> 8 -> 10 closes in fast; M=10 is good to ~5e-7, far below the MC error
+    e6, e8, e10 = (H.exact_mean_energy_L2(0.45, M) for M in (6, 8, 10))
+    assert abs(e8 - e10) < 0.1 * abs(e6 - e8) and abs(e8 - e10) < 5e-4
+    assert abs(e10 - (-12.961145712)) < 2e-6                   # SURVEY.md O9 (3-D Bessel quadrature) cross-check
+
+
+@pytest.mark.parametrize("with_or", [False, True])
+def test_O9_L2_mean_energy_against_brute_force(oracle_mod, with_or):
+    beta, R, T, burn = 0.45, 64, 6000, 50
+    want = H.exact_mean_energy_L2(beta, 10)
+    o = oracle_mod.XYOracle(2, R, np.full(R, beta), SEED + (1 if with_or else 0))
+    o.init_random()
+    E = np.empty((T, R))
+    for k in range(burn + T):
+        o.metropolis_sweep()
+        if with_or:
+            o.overrelax_sweep()
+        if k >= burn:
+            E[k - burn] = o.measure()[:, 0]
+    mean, err = H.mean_and_err_over_replicas(E)
+    assert err < 0.03
+    assert abs(mean - want) < 4 * err, (mean, want, err)
+
+
+# ------------------------------------------------------------------- O10/O11 exchange ----
+def test_O10_pt_equal_betas_swaps_every_attempted_pair(oracle_mod):
+    R = 7
+    o = oracle_mod.XYOracle(4, R, np.full(R, 0.45), SEED)
+    o.init_random()
+    perm = list(range(R))
+    for t in range(5):
+        o.pt_exchange()
+        for k in range(t & 1, R - 1, 2):
+            perm[k], perm[k + 1] = perm[k + 1], perm[k]
+        assert list(o.get_perm()) == perm
+        assert o.get_counters()[2] == t + 1
+    # R = 1 is a no-op
+    o1 = oracle_mod.XYOracle(4, 1, [0.45], SEED)
+    o1.init_random()
+    o1.pt_exchange()
+    assert list(o1.get_perm()) == [0]
+
+
+def test_pt_labels_follow_the_permutation_and_eq3_sign(oracle_mod):
+    R = 4
+    betas = np.array([0.2, 0.4, 0.6, 0.8])
+    o = oracle_mod.XYOracle(4, R, betas, SEED)
+    o.init_random()
+    # Eq. 3: a cold-labelled replica holding a much HIGHER energy than its hot neighbour always swaps;
+    # the reverse arrangement (already "sorted") swaps with probability exp(-|dbeta dE|) ~ 0.
+    tr = o.enable_trace(pt=True)
+    E = np.array([-100.0, +100.0, -100.0, +100.0])     # rank0(beta .2) E=-100, rank1(beta .4) E=+100 -> swap
+    o.pt_exchange(E)
+    assert list(o.get_perm()) == [1, 0, 3, 2]
+    assert np.allclose(tr["pt_p"][[0, 2]], np.exp(0.2 * 200.0))
+    assert np.allclose(o.get_beta_of_slot(), [0.4, 0.2, 0.8, 0.6])
+    o.set_counters([0, 0, 0])
+    o.pt_exchange(E)                                    # now rank0 holds slot1 (E=+100): sorted, no swap
+    assert list(o.get_perm()) == [1, 0, 3, 2]
+    assert np.allclose(tr["pt_p"][[0, 2]], np.exp(-0.2 * 200.0))
+    _, pt_acc = o.get_accept_counts()
+    assert list(pt_acc) == [1, 0, 1]
+
+
+def test_O11_pt_leaves_per_temperature_energy_unchanged(oracle_mod):
+    L, R, T, burn = 4, 4, 2500, 100
+    betas = np.array([0.40, 0.45, 0.50, 0.55])
+    n_copy = 6
+    res = {}
+    for with_pt in (False, True):
+        series = []
+        for copy in range(n_copy):
+            o = oracle_mod.XYOracle(L, R, betas, SEED + 10 * copy + (1 if with_pt else 0))
+            o.init_random()
+            E = np.empty((T, R))
+            for k in range(burn + T):
+                o.metropolis_sweep()
+                o.overrelax_sweep()
+                obs = o.measure()                       # indexed by rank
+                if with_pt:
+                    o.pt_exchange()
+                if k >= burn:
+                    E[k - burn] = obs[:, 0]
+            series.append(E.mean(axis=0))
+            if with_pt:
+                assert o.get_accept_counts()[1].sum() > 0.3 * T   # swaps do happen
+        s = np.array(series)
+        res[with_pt] = (s.mean(axis=0), s.std(axis=0, ddof=1) / np.sqrt(n_copy))
+    for k in range(R):
+        d = res[True][0][k] - res[False][0][k]
+        e = np.hypot(res[True][1][k], res[False][1][k])
+        assert abs(d) < 4 * e + 0.05, (k, d, e)
+    assert np.all(np.diff(res[True][0]) < 0)                      # colder ranks have lower energy
+
+
+# ------------------------------------------------------------------------- plumbing -----
+def test_result_is_independent_of_thread_count_and_active_slots(oracle_mod):
+    L, R = 6, 5
+    betas = inputs.beta_ladder(0.44, 0.47, R)
+    outs = []
+    for threads in (1, 3):
+        o = oracle_mod.XYOracle(L, R, betas, SEED, threads=threads)
+        o.init_random()
+        for _ in range(3):
+            o.mcs()
+        outs.append((o.get_state(), o.get_perm(), o.measure()))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    assert np.array_equal(outs[0][2], outs[1][2])
+    # a sweep restricted to slots {1,3} equals the full sweep on those slots and leaves the rest alone
+    a = oracle_mod.XYOracle(L, R, betas, SEED)
+    b = oracle_mod.XYOracle(L, R, betas, SEED)
+    a.init_random(); b.init_random()
+    s0 = a.get_state()
+    a.metropolis_sweep(); a.overrelax_sweep()
+    b.set_active_slots([1, 3])
+    b.metropolis_sweep(); b.overrelax_sweep()
+    sa, sb = a.get_state(), b.get_state()
+    assert np.array_equal(sa[[1, 3]], sb[[1, 3]]) and np.array_equal(sb[[0, 2, 4]], s0[[0, 2, 4]])
+
+
+def test_create_rejects_bad_arguments(oracle_mod):
+    for L, R, betas in ((3, 1, [0.4]), (0, 1, [0.4]), (4, 0, []), (4, 1, [float("nan")])):
+        with pytest.raises(ValueError):
+            oracle_mod.XYOracle(L, R, np.array(betas, dtype=np.float64).reshape(R), SEED)
+
+
+def test_O12_soft_physics_near_beta_c(oracle_mod):
+    """Gross-error check only (not parity): acceptance ~0.55 and E/N ~ -0.98 near beta_c."""
+    L, R = 12, 4
+    o = oracle_mod.XYOracle(L, R, np.full(R, 0.4542), SEED, threads=4)
+    o.init_random()
+    for _ in range(60):
+        o.metropolis_sweep(); o.overrelax_sweep()
+    a0 = o.get_accept_counts()[0].copy()
+    E = []
+    for _ in range(40):
+        o.metropolis_sweep(); o.overrelax_sweep()
+        E.append(o.measure()[:, 0].mean() / L ** 3)
+    acc = (o.get_accept_counts()[0] - a0).mean() / (40 * L ** 3)
+    assert 0.45 < acc < 0.65
+    assert -1.10 < np.mean(E) < -0.90
