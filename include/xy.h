@@ -1,0 +1,176 @@
+/* xy.h -- C ABI of the B200-native Monte Carlo step of the 3-D classical XY model
+ *
+ *     H = - sum_<ij> cos(theta_i - theta_j)        L x L x L periodic cubic lattice, J = k_B = 1
+ *
+ * over R parallel-tempering replicas, after arXiv:1211.0780 (cited as P:<line of PAPER.md>).
+ * One Monte Carlo step is
+ *
+ *     xy_metropolis_sweep -> xy_overrelax_sweep -> xy_measure -> xy_pt_exchange
+ *
+ * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.  The
+ * readings of the paper that these calls implement (proposal rule, colour order, RNG keying,
+ * pair selection, ...) are listed in DESIGN.md section 2 (R1..R17).
+ *
+ * Vocabulary.  N = L^3 sites.  A *slot* r is a physical spin array (it never moves); a *rank*
+ * k is an index into the caller's betas[] (a temperature).  Replica exchange permutes which
+ * slot carries which rank (slot_at_rank), never the spins (R11).  Natural layout means
+ * float theta[R][L][L][L] indexed [slot][z][y][x], x fastest, angles in radians in [0, 2 pi].
+ * Inside the library the state is colour-split: colour = (x+y+z)&1, 0 = black (updated
+ * first, R3); theta_c[slot][z][y][x>>1], two arrays of R*N/2 floats.
+ *
+ * Conventions.  Functions returning int return XY_OK (0) or a negative XY_ERR_*; they never
+ * throw, abort or print.  xy_last_error() gives a thread-local message for the last failing
+ * call.  Pointers are HOST pointers unless the parameter says "device".  A context is not
+ * thread-safe.  All device work is enqueued on the attached stream, in call order; only calls
+ * that return host data synchronise it.  L must be a multiple of 8 (128-bit rows), R >= 1.
+ */
+#ifndef XY_H_
+#define XY_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct xy_ctx xy_ctx;
+
+enum {
+    XY_OK = 0,
+    XY_ERR_INVALID_ARG = -1,  /* bad L/R/pointer/beta/option; nothing was enqueued             */
+    XY_ERR_CUDA = -2,         /* a CUDA call failed (message in xy_last_error)                 */
+    XY_ERR_NOT_ATTACHED = -3, /* the context has no device buffers yet (call xy_attach)        */
+    XY_ERR_NO_DEVICE = -4     /* no usable sm_100 device: the library never falls back to CPU  */
+};
+
+#define XY_NUM_OBS 5 /* E, Mx, My, |M|^2, |M|^4 */
+
+/* Tunables for xy_set_option (all optional; defaults are chosen from L and R). */
+enum {
+    XY_OPT_TILE_Y = 1,     /* rows of one colour per thread block (must divide L, TILE_Y*L/8 <= 1024) */
+    XY_OPT_TILE_Z = 2,     /* planes a thread block marches through (must divide L)                  */
+    XY_OPT_TRACE = 3,      /* 1: xy_metropolis_sweep also records its fast-path acceptance probability
+                              per site (test hook; allocates R*N floats inside the library)         */
+    XY_OPT_FUSED_MEASURE = 4 /* 1 (default): the white over-relaxation pass also accumulates the
+                              observables, so xy_measure after xy_overrelax_sweep reads no spins    */
+};
+
+/* ---- lifetime ------------------------------------------------------------------------------ */
+
+/* Creates the host-side description of one (L, R) system: copies betas[0..R-1] (rank order; need
+ * not be sorted -- adjacency for replica exchange is adjacency in this array), stores the
+ * Philox key `seed`, sets slot_at_rank[k] = k and all counters to 0.  Allocates nothing on the
+ * device.  Returns NULL on invalid arguments (L < 8 or L % 8 != 0, R < 1, NULL or non-finite
+ * betas); the reason is in xy_last_error().  [north_star: xy_create(L, R, betas, seed)] */
+xy_ctx* xy_create(int L, int R, const double* betas, uint64_t seed);
+
+/* Frees the context and whatever it allocated itself; attached caller-owned buffers and the
+ * stream are not touched.  NULL is allowed. */
+void xy_destroy(xy_ctx* ctx);
+
+/* Bytes of device memory a context of this shape needs: the colour-split state (R*N floats)
+ * and the workspace (reduction partials, results, permutation, beta labels, acceptance
+ * counters, one natural-layout staging slot).  0 on invalid (L, R). */
+size_t xy_state_bytes(int L, int R);
+size_t xy_workspace_bytes(int L, int R);
+
+/* Binds device memory and a stream.  d_state / d_workspace: DEVICE pointers, 256-byte aligned,
+ * of at least xy_state_bytes / xy_workspace_bytes, owned by the caller (PyTorch) and required to
+ * outlive the context; either may be NULL, in which case the library cudaMallocs and owns it.
+ * cuda_stream: a cudaStream_t (NULL = the legacy default stream).  Uploads the beta labels and
+ * the identity permutation; the spin state is undefined until xy_init_* or xy_set_state. */
+int xy_attach(xy_ctx* ctx, void* d_state, void* d_workspace, void* cuda_stream);
+
+/* ---- state (a0) ---------------------------------------------------------------------------- */
+
+/* Random start: theta[r][i] = fl32(2pi_f * u24(W[i&3])), W = Philox4x32-10(key = seed,
+ * counter = (i>>2, r, 0, stream 0)), i = x + L*(y + L*z)  [configs: "random-start angles from
+ * seed"; R12, R17].  Ordered start: every angle = theta0 [config 4].  Both reset the cached
+ * observables; neither touches counters or the permutation. */
+int xy_init_random(xy_ctx* ctx);
+int xy_init_ordered(xy_ctx* ctx, float theta0);
+
+/* Copies a natural-layout configuration in / out (R*N floats).  on_device = 0: `natural` is a
+ * host pointer (pinned memory makes the copy asynchronous-capable; the call synchronises
+ * before returning for xy_get_state, and before the host buffer may be reused for
+ * xy_set_state); on_device = 1: a device pointer readable from the attached stream, no
+ * synchronisation.  The layout conversion runs in a kernel. */
+int xy_set_state(xy_ctx* ctx, const float* natural, int on_device);
+int xy_get_state(xy_ctx* ctx, float* natural, int on_device);
+
+/* ---- the Monte Carlo step (a2..a5) ----------------------------------------------------------- */
+
+/* One checkerboard Metropolis sweep over all R slots: every black site, then every white site
+ * [P:30, Fig. 2 P:36].  For site i of slot r with local field h = sum over the six neighbours
+ * of (cos, sin) [P:23-28 Eq. 1]:  W = Philox(counter = (i>>2, r, n_met, 1 + colour)),
+ * p = (i>>1)&1, theta' = fl32(2pi_f * u24(W[2p])), dE = -h.(S(theta') - S(theta)),
+ * accept iff u24(W[2p+1]) < exp(-fl32(beta_of_slot[r]) * dE)  [R1, R2, R12, R13].
+ * The decision is taken in fp32 fast arithmetic when it is clear and re-evaluated in fp64
+ * from the stored angles when |u - p_fast| < 2^-14, so it equals the fp64 definition
+ * (DESIGN.md section 6).  Accepted angles are bit-identical to the definition.  ++n_met. */
+int xy_metropolis_sweep(xy_ctx* ctx);
+
+/* One checkerboard over-relaxation sweep, black then white: theta' = 2*atan2(h_y, h_x) - theta
+ * reduced to [0, 2pi); unchanged if h = 0  [P:38-43 Eq. 2; R4-R7].  fp32 arithmetic with a
+ * stated field error.  With XY_OPT_FUSED_MEASURE the white pass also
+ * produces the observables of the new state.  ++n_or. */
+int xy_overrelax_sweep(xy_ctx* ctx);
+
+/* Observables of the current state, out[R][5] = E, Mx, My, |M|^2, |M|^4 indexed by RANK k
+ * [P:52-56 Eqs. 4-5; E_n of Eq. 3; R14, R15]: E = -sum_bonds cos(theta_i - theta_j)
+ * (3N bonds), Mx = sum cos, My = sum sin; fp32 site terms, fp64 fixed-order accumulation
+ * (deterministic run to run).  out: host pointer, R*5 doubles, written after a stream
+ * synchronise; NULL = only enqueue the reduction (results stay on the device for
+ * xy_pt_exchange).  Re-uses cached results when the state has not changed since they were
+ * produced. */
+int xy_measure(xy_ctx* ctx, double* out);
+
+/* One replica exchange [P:45-50 Eq. 3; R8-R11]: for k = n_pt mod 2, k+2, ... with k+1 < R,
+ * a = slot_at_rank[k], b = slot_at_rank[k+1], u = W[0] * 2^-32 with
+ * W = Philox(counter = (k, 0, n_pt, 3)); accept iff u < exp((betas[k]-betas[k+1])*(E_a-E_b)),
+ * in fp64; on accept the two slots exchange their rank / beta label.  Uses the cached
+ * energies, running the reduction first if they are stale.  ++n_pt. */
+int xy_pt_exchange(xy_ctx* ctx);
+
+/* n_mcs repetitions of (Metropolis sweep, over-relaxation sweep, measure, PT exchange) [P:30],
+ * enqueued without host synchronisation.  series: DEVICE pointer to n_mcs*R*5 doubles that
+ * receives the by-rank observables of every step (measured before that step's exchange, R14),
+ * or NULL. */
+int xy_mcs(xy_ctx* ctx, int n_mcs, double* d_series);
+
+/* ---- bookkeeping ----------------------------------------------------------------------------- */
+
+int xy_get_perm(xy_ctx* ctx, int* slot_at_rank /* R, out */);         /* synchronises */
+int xy_set_perm(xy_ctx* ctx, const int* slot_at_rank /* R, a permutation */);
+int xy_get_beta_of_slot(xy_ctx* ctx, double* beta_of_slot /* R, out */); /* synchronises */
+int xy_get_counters(xy_ctx* ctx, uint32_t counters[3] /* n_met, n_or, n_pt */);
+int xy_set_counters(xy_ctx* ctx, const uint32_t counters[3]);
+/* Accepted Metropolis proposals per SLOT and accepted swaps per pair (k, k+1) since attach;
+ * either pointer may be NULL.  Synchronises. */
+int xy_get_accept_counts(xy_ctx* ctx, uint64_t* met_acc /* R */, uint64_t* pt_acc /* R-1 */);
+/* Number of Metropolis decisions that took the fp64 re-evaluation since attach.  Synchronises. */
+int xy_get_exact_path_count(xy_ctx* ctx, uint64_t* n);
+int xy_set_option(xy_ctx* ctx, int option, int value);
+int xy_get_option(xy_ctx* ctx, int option, int* value);
+/* Number of kernels this context has launched since attach (bench.py's gpu_launches). */
+int xy_get_launch_count(xy_ctx* ctx, uint64_t* n);
+int xy_synchronize(xy_ctx* ctx);
+const char* xy_last_error(void);
+
+/* ---- test hooks (stated-error measurements; not part of the Monte Carlo step) ---------------- */
+
+/* With XY_OPT_TRACE = 1: the fast-path acceptance probability min(p_fast, FLT_MAX) of every site
+ * in the last xy_metropolis_sweep, natural layout, host pointer, R*N floats.  Synchronises. */
+int xy_debug_get_trace(xy_ctx* ctx, float* natural);
+/* Evaluate the kernels' device math on n DEVICE floats (stream = cudaStream_t or NULL):
+ * fast sin/cos of x[i]; fast atan2(y[i], x[i]) in [0, 2pi); Philox words of n counters. */
+int xy_debug_sincos(const float* d_x, float* d_cos, float* d_sin, size_t n, void* cuda_stream);
+int xy_debug_atan2(const float* d_y, const float* d_x, float* d_phi, size_t n, void* cuda_stream);
+int xy_debug_philox(const uint32_t* d_ctr /* n*4 */, uint32_t key0, uint32_t key1,
+                    uint32_t* d_out /* n*4 */, size_t n, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* XY_H_ */

@@ -1,0 +1,494 @@
+// xy_api.cu -- the C ABI of include/xy.h: host-side bookkeeping and kernel launches.
+// Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -shared -Xcompiler -fPIC
+#include "../../include/xy.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "xy_kernels.cuh"
+
+using namespace xyk;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) return fail(XY_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); \
+    } while (0)
+
+size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+bool shape_ok(int L, int R) { return L >= 8 && L % 8 == 0 && L <= 1024 && R >= 1 && R <= 65535; }
+size_t max_tiles(int L) { return (size_t)(L / 8) * (size_t)(L / 2); }
+
+struct WsLayout {
+    size_t obs_rank, obs_slot, partials, betas, beta_of_slot, beta32, slot_at_rank, met_acc, pt_acc, exact, stage, total;
+};
+WsLayout ws_layout(int L, int R) {
+    WsLayout w;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+    w.obs_rank = take((size_t)R * 5 * 8);
+    w.obs_slot = take((size_t)R * 5 * 8);
+    w.partials = take((size_t)R * max_tiles(L) * 3 * 8);
+    w.betas = take((size_t)R * 8);
+    w.beta_of_slot = take((size_t)R * 8);
+    w.beta32 = take((size_t)R * 4);
+    w.slot_at_rank = take((size_t)R * 4);
+    w.met_acc = take((size_t)R * 8);
+    w.pt_acc = take((size_t)R * 8);
+    w.exact = take(8);
+    w.stage = take((size_t)L * L * L * 4);
+    w.total = o;
+    return w;
+}
+
+}  // namespace
+
+struct xy_ctx {
+    int L = 0, R = 0;
+    size_t N = 0, half_n = 0;
+    uint64_t seed = 0;
+    std::vector<double> betas;
+    PhiloxKeys keys;
+    uint32_t n_met = 0, n_or = 0, n_pt = 0;
+    // device
+    bool attached = false;
+    float* d_state = nullptr; bool own_state = false;
+    char* d_ws = nullptr; bool own_ws = false;
+    cudaStream_t stream = nullptr;
+    WsLayout ws;
+    float* d_trace = nullptr;
+    // options
+    int TY = 0, TZ = 0, trace = 0, fused = 0;
+    // cache state
+    bool partials_valid = false, rank_valid = false;
+    uint64_t launches = 0;
+
+    float* colour(int c) const { return d_state + (size_t)c * R * half_n; }
+    template <class T> T* ws_ptr(size_t off) const { return reinterpret_cast<T*>(d_ws + off); }
+};
+
+namespace {
+
+void default_tiles(int L, int R, int& TY, int& TZ) {
+    const int W4 = L / 8;
+    TY = 8;
+    for (int t = 8; t <= L; ++t)
+        if (L % t == 0 && t * W4 <= 320) TY = t;
+    // march length: long enough to amortise the two halo planes, short enough for >= ~4 waves of CTAs
+    TZ = L;
+    const long want = 4L * 148 * 3;
+    for (int t = L; t >= 8; --t) {
+        if (L % t) continue;
+        TZ = t;
+        if ((long)R * (L / TY) * (L / t) >= want) break;
+    }
+    if (TZ < 8) TZ = L < 8 ? L : 8;
+}
+
+bool tiles_ok(int L, int TY, int TZ) {
+    return TY >= 2 && TZ >= 2 && L % TY == 0 && L % TZ == 0 && TY * (L / 8) <= 512 &&
+           (size_t)32 * (TY + 2) * (L / 2) <= 200 * 1024;
+}
+
+template <int MODE, bool TRACE>
+int launch_sweep(xy_ctx* c, const SweepParams& P) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        CK(cudaFuncSetAttribute(sweep_kernel<MODE, TRACE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        attr_set = true;
+    }
+    const size_t smem = (size_t)32 * (P.TY + 2) * P.W;
+    int threads = P.nItems > 2 * P.W4 ? P.nItems : 2 * P.W4;
+    threads = (threads + 31) / 32 * 32;
+    dim3 grid(P.nTY * P.nTZ, c->R);
+    sweep_kernel<MODE, TRACE><<<grid, threads, smem, c->stream>>>(P);
+    CK(cudaGetLastError());
+    ++c->launches;
+    return XY_OK;
+}
+
+SweepParams base_params(xy_ctx* c, int colour) {
+    SweepParams P;
+    memset(&P, 0, sizeof(P));
+    P.own = c->colour(colour);
+    P.other = c->colour(1 - colour);
+    P.L = c->L; P.W = c->L / 2; P.W4 = c->L / 8;
+    P.TY = c->TY; P.TZ = c->TZ; P.nTY = c->L / c->TY; P.nTZ = c->L / c->TZ;
+    P.colour = colour;
+    P.nItems = P.TY * P.W4;
+    P.half_n = c->half_n;
+    P.keys = c->keys;
+    P.beta32_of_slot = c->ws_ptr<float>(c->ws.beta32);
+    P.met_acc = c->ws_ptr<unsigned long long>(c->ws.met_acc);
+    P.exact_count = c->ws_ptr<unsigned long long>(c->ws.exact);
+    P.partials = c->ws_ptr<double>(c->ws.partials);
+    return P;
+}
+
+int need(xy_ctx* c) {
+    if (!c) return fail(XY_ERR_INVALID_ARG, "NULL context");
+    if (!c->attached) return fail(XY_ERR_NOT_ATTACHED, "context has no device buffers: call xy_attach first");
+    return XY_OK;
+}
+
+int upload_labels(xy_ctx* c, const int* perm) {
+    const int R = c->R;
+    std::vector<double> bos(R);
+    std::vector<float> b32(R);
+    std::vector<int> sar(R);
+    for (int k = 0; k < R; ++k) { sar[k] = perm ? perm[k] : k; bos[sar[k]] = c->betas[k]; b32[sar[k]] = (float)c->betas[k]; }
+    CK(cudaMemcpyAsync(c->ws_ptr<double>(c->ws.betas), c->betas.data(), R * 8, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->ws_ptr<double>(c->ws.beta_of_slot), bos.data(), R * 8, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->ws_ptr<float>(c->ws.beta32), b32.data(), R * 4, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->ws_ptr<int>(c->ws.slot_at_rank), sar.data(), R * 4, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));     // the host vectors die here
+    c->rank_valid = false;
+    return XY_OK;
+}
+
+int grid_for(size_t n_items, int threads) {
+    size_t b = (n_items + threads - 1) / threads;
+    const size_t cap = 148 * 16;
+    return (int)(b < 1 ? 1 : (b > cap ? cap : b));
+}
+
+int run_measure(xy_ctx* c, double* d_series_row) {
+    if (!c->partials_valid) {
+        SweepParams P = base_params(c, 1);     // own = white, staged = black
+        int rc = launch_sweep<MODE_MEASURE, false>(c, P);
+        if (rc) return rc;
+        c->partials_valid = true;
+        c->rank_valid = false;
+    }
+    if (!c->rank_valid || d_series_row) {
+        const int n_tiles = (c->L / c->TY) * (c->L / c->TZ);
+        measure_finalize_kernel<<<c->R, 128, 0, c->stream>>>(c->ws_ptr<double>(c->ws.partials), n_tiles,
+                                                             c->ws_ptr<int>(c->ws.slot_at_rank),
+                                                             c->ws_ptr<double>(c->ws.obs_rank),
+                                                             c->ws_ptr<double>(c->ws.obs_slot), d_series_row);
+        CK(cudaGetLastError());
+        ++c->launches;
+        c->rank_valid = true;
+    }
+    return XY_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* xy_last_error(void) { return g_err; }
+
+xy_ctx* xy_create(int L, int R, const double* betas, uint64_t seed) {
+    if (!shape_ok(L, R)) { fail(XY_ERR_INVALID_ARG, "xy_create: need L %% 8 == 0, 8 <= L <= 1024, 1 <= R <= 65535 (got L=%d R=%d)", L, R); return nullptr; }
+    if (!betas) { fail(XY_ERR_INVALID_ARG, "xy_create: betas is NULL"); return nullptr; }
+    for (int k = 0; k < R; ++k)
+        if (!std::isfinite(betas[k])) { fail(XY_ERR_INVALID_ARG, "xy_create: betas[%d] is not finite", k); return nullptr; }
+    xy_ctx* c = new xy_ctx;
+    c->L = L; c->R = R; c->N = (size_t)L * L * L; c->half_n = c->N / 2; c->seed = seed;
+    c->betas.assign(betas, betas + R);
+    c->keys = philox_round_keys((uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32));
+    c->ws = ws_layout(L, R);
+    default_tiles(L, R, c->TY, c->TZ);
+    return c;
+}
+
+void xy_destroy(xy_ctx* c) {
+    if (!c) return;
+    if (c->own_state && c->d_state) cudaFree(c->d_state);
+    if (c->own_ws && c->d_ws) cudaFree(c->d_ws);
+    if (c->d_trace) cudaFree(c->d_trace);
+    delete c;
+}
+
+size_t xy_state_bytes(int L, int R) { return shape_ok(L, R) ? (size_t)R * L * L * L * 4 : 0; }
+size_t xy_workspace_bytes(int L, int R) { return shape_ok(L, R) ? ws_layout(L, R).total : 0; }
+
+int xy_attach(xy_ctx* c, void* d_state, void* d_workspace, void* cuda_stream) {
+    if (!c) return fail(XY_ERR_INVALID_ARG, "NULL context");
+    if (c->attached) return fail(XY_ERR_INVALID_ARG, "xy_attach: context is already attached");
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) {
+        cudaGetLastError();
+        return fail(XY_ERR_NO_DEVICE, "xy_attach: no CUDA device; this library has no CPU fallback");
+    }
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major < 10) return fail(XY_ERR_NO_DEVICE, "xy_attach: device %s is sm_%d%d; built for sm_100a only", prop.name, prop.major, prop.minor);
+    if (((uintptr_t)d_state | (uintptr_t)d_workspace) & 255u) return fail(XY_ERR_INVALID_ARG, "xy_attach: buffers must be 256-byte aligned");
+    c->stream = (cudaStream_t)cuda_stream;
+    if (d_state) { c->d_state = (float*)d_state; c->own_state = false; }
+    else { CK(cudaMalloc(&c->d_state, xy_state_bytes(c->L, c->R))); c->own_state = true; }
+    if (d_workspace) { c->d_ws = (char*)d_workspace; c->own_ws = false; }
+    else { CK(cudaMalloc(&c->d_ws, c->ws.total)); c->own_ws = true; }
+    CK(cudaMemsetAsync(c->d_ws, 0, c->ws.stage, c->stream));     // everything but the staging slot
+    c->attached = true;
+    c->partials_valid = c->rank_valid = false;
+    c->launches = 0;
+    return upload_labels(c, nullptr);
+}
+
+int xy_init_random(xy_ctx* c) {
+    if (int rc = need(c)) return rc;
+    const size_t n_quads = (size_t)c->R * c->L * c->L * (c->L / 4);
+    init_random_kernel<<<grid_for(n_quads, 256), 256, 0, c->stream>>>(c->colour(0), c->colour(1), c->L, c->R, c->keys);
+    CK(cudaGetLastError());
+    ++c->launches;
+    c->partials_valid = false;
+    return XY_OK;
+}
+
+int xy_init_ordered(xy_ctx* c, float theta0) {
+    if (int rc = need(c)) return rc;
+    const size_t n = (size_t)c->R * c->N;
+    fill_kernel<<<grid_for(n, 256), 256, 0, c->stream>>>(c->d_state, n, theta0);
+    CK(cudaGetLastError());
+    ++c->launches;
+    c->partials_valid = false;
+    return XY_OK;
+}
+
+static int convert_state(xy_ctx* c, float* black, float* white, float* natural, int on_device, bool to_split) {
+    const int L = c->L;
+    const size_t per_slot = (size_t)L * L * (L / 8);
+    if (on_device) {
+        const size_t n = per_slot * c->R;
+        if (to_split) convert_kernel<true><<<grid_for(n, 256), 256, 0, c->stream>>>(natural, black, white, L, c->R, 0);
+        else convert_kernel<false><<<grid_for(n, 256), 256, 0, c->stream>>>(natural, black, white, L, c->R, 0);
+        CK(cudaGetLastError());
+        ++c->launches;
+        return XY_OK;
+    }
+    float* stage = c->ws_ptr<float>(c->ws.stage);
+    for (int r = 0; r < c->R; ++r) {            // one natural slot at a time through the staging buffer
+        float* h = natural + (size_t)r * c->N;
+        if (to_split) {
+            CK(cudaMemcpyAsync(stage, h, c->N * 4, cudaMemcpyHostToDevice, c->stream));
+            convert_kernel<true><<<grid_for(per_slot, 256), 256, 0, c->stream>>>(stage, black, white, L, 1, r);
+        } else {
+            convert_kernel<false><<<grid_for(per_slot, 256), 256, 0, c->stream>>>(stage, black, white, L, 1, r);
+            CK(cudaMemcpyAsync(h, stage, c->N * 4, cudaMemcpyDeviceToHost, c->stream));
+        }
+        CK(cudaGetLastError());
+        ++c->launches;
+    }
+    CK(cudaStreamSynchronize(c->stream));
+    return XY_OK;
+}
+
+int xy_set_state(xy_ctx* c, const float* natural, int on_device) {
+    if (int rc = need(c)) return rc;
+    if (!natural) return fail(XY_ERR_INVALID_ARG, "xy_set_state: NULL pointer");
+    c->partials_valid = false;
+    return convert_state(c, c->colour(0), c->colour(1), const_cast<float*>(natural), on_device, true);
+}
+
+int xy_get_state(xy_ctx* c, float* natural, int on_device) {
+    if (int rc = need(c)) return rc;
+    if (!natural) return fail(XY_ERR_INVALID_ARG, "xy_get_state: NULL pointer");
+    return convert_state(c, c->colour(0), c->colour(1), natural, on_device, false);
+}
+
+int xy_metropolis_sweep(xy_ctx* c) {
+    if (int rc = need(c)) return rc;
+    if (c->trace && !c->d_trace) CK(cudaMalloc(&c->d_trace, (size_t)c->R * c->N * 4));
+    for (int colour = 0; colour < 2; ++colour) {
+        SweepParams P = base_params(c, colour);
+        P.sweep = c->n_met;
+        P.trace = c->d_trace;
+        int rc = c->trace ? launch_sweep<MODE_MET, true>(c, P) : launch_sweep<MODE_MET, false>(c, P);
+        if (rc) return rc;
+    }
+    ++c->n_met;
+    c->partials_valid = false;
+    return XY_OK;
+}
+
+int xy_overrelax_sweep(xy_ctx* c) {
+    if (int rc = need(c)) return rc;
+    for (int colour = 0; colour < 2; ++colour) {
+        SweepParams P = base_params(c, colour);
+        int rc = launch_sweep<MODE_OR, false>(c, P);
+        if (rc) return rc;
+    }
+    ++c->n_or;
+    c->partials_valid = false;
+    return XY_OK;
+}
+
+int xy_measure(xy_ctx* c, double* out) {
+    if (int rc = need(c)) return rc;
+    if (int rc = run_measure(c, nullptr)) return rc;
+    if (out) {
+        CK(cudaMemcpyAsync(out, c->ws_ptr<double>(c->ws.obs_rank), (size_t)c->R * 5 * 8, cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaStreamSynchronize(c->stream));
+    }
+    return XY_OK;
+}
+
+int xy_pt_exchange(xy_ctx* c) {
+    if (int rc = need(c)) return rc;
+    if (int rc = run_measure(c, nullptr)) return rc;
+    const int pairs = c->R / 2 + 1;
+    pt_exchange_kernel<<<(pairs + 127) / 128, 128, 0, c->stream>>>(
+        c->R, c->n_pt, c->keys, c->ws_ptr<double>(c->ws.betas), c->ws_ptr<double>(c->ws.obs_slot),
+        c->ws_ptr<int>(c->ws.slot_at_rank), c->ws_ptr<double>(c->ws.beta_of_slot), c->ws_ptr<float>(c->ws.beta32),
+        c->ws_ptr<unsigned long long>(c->ws.pt_acc));
+    CK(cudaGetLastError());
+    ++c->launches;
+    ++c->n_pt;
+    c->rank_valid = false;
+    return XY_OK;
+}
+
+int xy_mcs(xy_ctx* c, int n_mcs, double* d_series) {
+    if (int rc = need(c)) return rc;
+    if (n_mcs < 0) return fail(XY_ERR_INVALID_ARG, "xy_mcs: n_mcs < 0");
+    for (int t = 0; t < n_mcs; ++t) {
+        if (int rc = xy_metropolis_sweep(c)) return rc;
+        if (int rc = xy_overrelax_sweep(c)) return rc;
+        if (int rc = run_measure(c, d_series ? d_series + (size_t)t * c->R * 5 : nullptr)) return rc;
+        if (int rc = xy_pt_exchange(c)) return rc;
+    }
+    return XY_OK;
+}
+
+int xy_get_perm(xy_ctx* c, int* p) {
+    if (int rc = need(c)) return rc;
+    if (!p) return fail(XY_ERR_INVALID_ARG, "xy_get_perm: NULL pointer");
+    CK(cudaMemcpyAsync(p, c->ws_ptr<int>(c->ws.slot_at_rank), c->R * 4, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return XY_OK;
+}
+
+int xy_set_perm(xy_ctx* c, const int* p) {
+    if (int rc = need(c)) return rc;
+    if (!p) return fail(XY_ERR_INVALID_ARG, "xy_set_perm: NULL pointer");
+    std::vector<char> seen(c->R, 0);
+    for (int k = 0; k < c->R; ++k) {
+        if (p[k] < 0 || p[k] >= c->R || seen[p[k]]) return fail(XY_ERR_INVALID_ARG, "xy_set_perm: not a permutation of 0..R-1");
+        seen[p[k]] = 1;
+    }
+    return upload_labels(c, p);
+}
+
+int xy_get_beta_of_slot(xy_ctx* c, double* b) {
+    if (int rc = need(c)) return rc;
+    if (!b) return fail(XY_ERR_INVALID_ARG, "xy_get_beta_of_slot: NULL pointer");
+    CK(cudaMemcpyAsync(b, c->ws_ptr<double>(c->ws.beta_of_slot), c->R * 8, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return XY_OK;
+}
+
+int xy_get_counters(xy_ctx* c, uint32_t n[3]) {
+    if (!c || !n) return fail(XY_ERR_INVALID_ARG, "xy_get_counters: NULL argument");
+    n[0] = c->n_met; n[1] = c->n_or; n[2] = c->n_pt;
+    return XY_OK;
+}
+
+int xy_set_counters(xy_ctx* c, const uint32_t n[3]) {
+    if (!c || !n) return fail(XY_ERR_INVALID_ARG, "xy_set_counters: NULL argument");
+    c->n_met = n[0]; c->n_or = n[1]; c->n_pt = n[2];
+    return XY_OK;
+}
+
+int xy_get_accept_counts(xy_ctx* c, uint64_t* met, uint64_t* pt) {
+    if (int rc = need(c)) return rc;
+    if (met) CK(cudaMemcpyAsync(met, c->ws_ptr<char>(c->ws.met_acc), c->R * 8, cudaMemcpyDeviceToHost, c->stream));
+    if (pt && c->R > 1) CK(cudaMemcpyAsync(pt, c->ws_ptr<char>(c->ws.pt_acc), (c->R - 1) * 8, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return XY_OK;
+}
+
+int xy_get_exact_path_count(xy_ctx* c, uint64_t* n) {
+    if (int rc = need(c)) return rc;
+    if (!n) return fail(XY_ERR_INVALID_ARG, "xy_get_exact_path_count: NULL pointer");
+    CK(cudaMemcpyAsync(n, c->ws_ptr<char>(c->ws.exact), 8, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return XY_OK;
+}
+
+int xy_set_option(xy_ctx* c, int option, int value) {
+    if (!c) return fail(XY_ERR_INVALID_ARG, "NULL context");
+    switch (option) {
+        case XY_OPT_TILE_Y:
+            if (!tiles_ok(c->L, value, c->TZ)) return fail(XY_ERR_INVALID_ARG, "XY_OPT_TILE_Y=%d invalid for L=%d", value, c->L);
+            c->TY = value; c->partials_valid = false; return XY_OK;
+        case XY_OPT_TILE_Z:
+            if (!tiles_ok(c->L, c->TY, value)) return fail(XY_ERR_INVALID_ARG, "XY_OPT_TILE_Z=%d invalid for L=%d", value, c->L);
+            c->TZ = value; c->partials_valid = false; return XY_OK;
+        case XY_OPT_TRACE: c->trace = value ? 1 : 0; return XY_OK;
+        case XY_OPT_FUSED_MEASURE: c->fused = value ? 1 : 0; return XY_OK;
+        default: return fail(XY_ERR_INVALID_ARG, "unknown option %d", option);
+    }
+}
+
+int xy_get_option(xy_ctx* c, int option, int* value) {
+    if (!c || !value) return fail(XY_ERR_INVALID_ARG, "NULL argument");
+    switch (option) {
+        case XY_OPT_TILE_Y: *value = c->TY; return XY_OK;
+        case XY_OPT_TILE_Z: *value = c->TZ; return XY_OK;
+        case XY_OPT_TRACE: *value = c->trace; return XY_OK;
+        case XY_OPT_FUSED_MEASURE: *value = c->fused; return XY_OK;
+        default: return fail(XY_ERR_INVALID_ARG, "unknown option %d", option);
+    }
+}
+
+int xy_get_launch_count(xy_ctx* c, uint64_t* n) {
+    if (!c || !n) return fail(XY_ERR_INVALID_ARG, "NULL argument");
+    *n = c->launches;
+    return XY_OK;
+}
+
+int xy_synchronize(xy_ctx* c) {
+    if (int rc = need(c)) return rc;
+    CK(cudaStreamSynchronize(c->stream));
+    return XY_OK;
+}
+
+int xy_debug_get_trace(xy_ctx* c, float* natural) {
+    if (int rc = need(c)) return rc;
+    if (!natural) return fail(XY_ERR_INVALID_ARG, "xy_debug_get_trace: NULL pointer");
+    if (!c->d_trace) return fail(XY_ERR_INVALID_ARG, "xy_debug_get_trace: no trace recorded (set XY_OPT_TRACE before the sweep)");
+    return convert_state(c, c->d_trace, c->d_trace + (size_t)c->R * c->half_n, natural, 0, false);
+}
+
+int xy_debug_sincos(const float* d_x, float* d_cos, float* d_sin, size_t n, void* stream) {
+    if (!d_x || !d_cos || !d_sin) return fail(XY_ERR_INVALID_ARG, "xy_debug_sincos: NULL pointer");
+    debug_sincos_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)stream>>>(d_x, d_cos, d_sin, n);
+    CK(cudaGetLastError());
+    return XY_OK;
+}
+
+int xy_debug_atan2(const float* d_y, const float* d_x, float* d_phi, size_t n, void* stream) {
+    if (!d_x || !d_y || !d_phi) return fail(XY_ERR_INVALID_ARG, "xy_debug_atan2: NULL pointer");
+    debug_atan2_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)stream>>>(d_y, d_x, d_phi, n);
+    CK(cudaGetLastError());
+    return XY_OK;
+}
+
+int xy_debug_philox(const uint32_t* d_ctr, uint32_t key0, uint32_t key1, uint32_t* d_out, size_t n, void* stream) {
+    if (!d_ctr || !d_out) return fail(XY_ERR_INVALID_ARG, "xy_debug_philox: NULL pointer");
+    debug_philox_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)stream>>>(d_ctr, philox_round_keys(key0, key1), d_out, n);
+    CK(cudaGetLastError());
+    return XY_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,136 @@
+// xy_device.cuh -- device-side building blocks of the XY Monte Carlo step (sm_100a).
+// In-register Philox4x32-10, uniforms, fast fp32 sin/cos/atan2/exp2 with stated errors, and the
+// fp64 re-evaluation of a Metropolis decision.  Shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace xyk {
+
+// ---------------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon et al., SC'11) -- north_star "generated in registers"; replaces the
+// Warp Generator of P:30.  The ten round keys depend only on the seed, so the host computes
+// them once and the kernels read them from the constant bank (no per-thread key schedule).
+// ---------------------------------------------------------------------------------------------
+struct PhiloxKeys { uint32_t k[20]; };
+
+constexpr uint32_t kPhiloxM0 = 0xD2511F53u, kPhiloxM1 = 0xCD9E8D57u;
+constexpr uint32_t kPhiloxW0 = 0x9E3779B9u, kPhiloxW1 = 0xBB67AE85u;
+
+__host__ inline PhiloxKeys philox_round_keys(uint32_t key0, uint32_t key1) {
+    PhiloxKeys K;
+    for (int r = 0; r < 10; ++r) { K.k[2 * r] = key0 + r * kPhiloxW0; K.k[2 * r + 1] = key1 + r * kPhiloxW1; }
+    return K;
+}
+
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              const PhiloxKeys& K, uint32_t (&out)[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)kPhiloxM0 * c0;      // IMAD.WIDE.U32
+        const uint64_t p1 = (uint64_t)kPhiloxM1 * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ K.k[2 * r];        // LOP3
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ K.k[2 * r + 1];
+        c1 = (uint32_t)p1; c3 = (uint32_t)p0; c0 = n0; c2 = n2;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+enum : uint32_t { kStreamInit = 0, kStreamMetBlack = 1, kStreamMetWhite = 2, kStreamPT = 3 };   // R12
+
+// ---------------------------------------------------------------------------------------------
+// Uniforms (R17).  u24(w) = (w >> 8) * 2^-24 is exact in fp32.  The proposal angle is
+// fl32(2pi_f * u24): because 2^-24 is a power of two, (float)(w>>8) * (2pi_f * 2^-24) rounds
+// once to exactly that value.
+// ---------------------------------------------------------------------------------------------
+constexpr float kTwoPiF = 6.2831855f;                                   // 0x40C90FDB
+constexpr float kTwoPiU24 = 6.2831855f * 5.9604644775390625e-08f;       // 2pi_f * 2^-24 (exact scaling)
+constexpr float kInvU24 = 5.9604644775390625e-08f;                      // 2^-24
+constexpr float kPiF = 3.14159274f;
+constexpr float kHalfPiF = 1.57079637f;
+
+__device__ __forceinline__ float word_to_angle(uint32_t w) { return (float)(w >> 8) * kTwoPiU24; }
+__device__ __forceinline__ float word_to_u24(uint32_t w) { return (float)(w >> 8) * kInvU24; }
+
+// ---------------------------------------------------------------------------------------------
+// Fast fp32 math.  Stated errors (measured by tests/test_gpu_parity.py::test_device_math_errors
+// against fp64 on [0, 2pi]):  sin/cos abs error <= 1.0e-6 (MUFU.SIN/COS after one FMUL by 1/2pi);
+// atan2 abs error <= 6e-7 rad; ex2.approx relative error <= 2^-22.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void fast_sincos(float x, float& s, float& c) {
+    s = __sinf(x);
+    c = __cosf(x);
+}
+
+__device__ __forceinline__ float fast_ex2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+__device__ __forceinline__ float fast_rcp(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// atan2(y, x) in [0, 2pi] for (x, y) != (0, 0): octant reduction to r = min/max in [0, 1], then a
+// degree-13 odd minimax polynomial (Remez fit, |error| <= 2.5e-7 in exact arithmetic).
+__device__ __forceinline__ float fast_atan2_pos(float y, float x) {
+    const float ax = fabsf(x), ay = fabsf(y);
+    const float mx = fmaxf(ax, ay), mn = fminf(ax, ay);
+    const float r = mn * fast_rcp(mx);
+    const float s = r * r;
+    float p = 0.006811792962253094f;
+    p = fmaf(p, s, -0.0336042195558548f);
+    p = fmaf(p, s, 0.07962366938591003f);
+    p = fmaf(p, s, -0.1323334276676178f);
+    p = fmaf(p, s, 0.19807815551757812f);
+    p = fmaf(p, s, -0.3331736922264099f);
+    p = fmaf(p, s, 0.9999961256980896f);
+    float a = p * r;
+    a = (ay > ax) ? (kHalfPiF - a) : a;
+    a = (x < 0.0f) ? (kPiF - a) : a;
+    a = (y < 0.0f) ? (kTwoPiF - a) : a;
+    return a;
+}
+
+// ---------------------------------------------------------------------------------------------
+// fp64 re-evaluation of one Metropolis decision from the STORED angles (not from the staged
+// fp32 sin/cos): the definition of include/xy.h, computed in double like the paper's Eq. 1
+// demands.  Taken by ~1e-4 of the decisions, so it is kept out of line.
+//   other: this slot's other-colour array [z][y][W];  par: x parity of this site's row,
+//   xh: x >> 1.  Neighbour order mirrors the definition: -x, -y, -z, +x, +y, +z.
+// ---------------------------------------------------------------------------------------------
+__device__ __noinline__ bool metropolis_exact(const float* __restrict__ other, int L, int W, int par,
+                                              int xh, int y, int z, float t_old, float t_new, float u,
+                                              float beta32) {
+    const int xm = par ? xh : (xh == 0 ? W - 1 : xh - 1);
+    const int xp = par ? (xh + 1 == W ? 0 : xh + 1) : xh;
+    const int ym = y == 0 ? L - 1 : y - 1, yp = y + 1 == L ? 0 : y + 1;
+    const int zm = z == 0 ? L - 1 : z - 1, zp = z + 1 == L ? 0 : z + 1;
+    const size_t row = (size_t)z * L + y;
+    const float nb[6] = {
+        other[row * W + xm], other[((size_t)z * L + ym) * W + xh], other[((size_t)zm * L + y) * W + xh],
+        other[row * W + xp], other[((size_t)z * L + yp) * W + xh], other[((size_t)zp * L + y) * W + xh] };
+    double hx = 0.0, hy = 0.0;
+#pragma unroll 1
+    for (int j = 0; j < 6; ++j) {
+        double s, c;
+        sincos((double)nb[j], &s, &c);
+        hx += c; hy += s;
+    }
+    double so, co, sn, cn;
+    sincos((double)t_old, &so, &co);
+    sincos((double)t_new, &sn, &cn);
+    const double dE = -(hx * (cn - co) + hy * (sn - so));
+    return (double)u < exp(-(double)beta32 * dE);
+}
+
+// Half-width of the window around p_fast inside which the decision is re-evaluated in fp64.
+// The fast path's |p_fast - p_exact| is bounded by beta*(|dh||dS| + |h||d(dS)|) + p*2^-22
+// ~ 0.46*(6e-6*2.9 + 6*2.9e-6) + 2.4e-7 < 1.7e-5 in the very worst case (every one of the 16
+// sin/cos errors at its 1e-6 maximum and aligned); 2^-14 = 6.1e-5 leaves a factor > 3.
+constexpr float kExactWindow = 6.103515625e-05f;
+
+}  // namespace xyk
