@@ -1,0 +1,277 @@
+#!/usr/bin/env python
+"""bench.py -- spin-updates/ns of one Monte Carlo step (MCS) of the 3-D XY model at L=160 x 64 replicas.
+
+A "step" is one pass of the whole hot path over all R replicas: checkerboard Metropolis sweep,
+checkerboard over-relaxation sweep, observable reduction, replica exchange.  One
+spin-update = one Metropolis attempt or one over-relaxation reflection of one site, so a step
+performs 2 * L^3 * R spin-updates.  Prints ONE JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 0..4]
+
+N > 1 (under torchrun): the path does not shard (north_star: one GPU) -- every rank runs an
+independent replica set of the same size ("replicas only", weak scaling), no data-path collective.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1211_0780_b200 import inputs  # noqa: E402  (no CUDA needed to import)
+
+METRIC = "spin-updates/ns per MCS at L=160x64 replicas"
+UNIT = "spin-updates/ns"
+BYTES_PER_UPDATE = 12          # colour-split layout: read own + other colour, write own
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
+# `ncu --set full` capture (profiles/), keyed by config name; None until captured.
+NCU_TRAFFIC_BYTES = {}
+try:
+    with open(os.path.join(ROOT, "profiles", "traffic.json.txt")) as _f:
+        NCU_TRAFFIC_BYTES = json.load(_f)
+except Exception:
+    pass
+
+
+def measured_peak_gbs():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons every 200 ms DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device_index):
+        self.rows, self.proc, self.thread = [], None, None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(device_index)],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()          # exactly the process started above
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        rows = [r for t, r in self.rows if t0 <= t <= t1 + 0.2 and len(r) >= 7] or [r for _, r in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "power_w_max": max(float(r[2]) for r in rows),
+                "samples": len(rows), "reasons": reasons}
+
+
+def combine_ranks(ms_local, units_local, dist=None, device="cpu"):
+    """max over ranks of the elapsed time, sum over ranks of the units processed (spin-updates)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(ms_local), float(units_local)
+    import torch
+    t = torch.tensor([float(ms_local)], dtype=torch.float64, device=device)
+    u = torch.tensor([float(units_local)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def oracle_sample_rate(cfg, n_slots, steps, warmup, threads):
+    """The CPU oracle, as it stands, on a bounded sample: full MCS of the first n_slots temperatures of cfg."""
+    from oracle import xy_oracle
+    betas = inputs.betas_of(cfg)[:n_slots]
+    ora = xy_oracle.XYOracle(cfg.L, n_slots, betas, inputs.SEED, threads=threads)
+    if cfg.start == "random":
+        ora.init_random()
+    else:
+        ora.init_ordered(0.0)
+    for _ in range(warmup):
+        ora.mcs()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        ora.mcs()
+    dt = time.perf_counter() - t0
+    updates = 2.0 * cfg.L ** 3 * n_slots * steps
+    return updates / dt * 1e-9, dt / steps * 1e3
+
+
+def run_reference(args, cfg):
+    """--impl reference: the oracle on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    cores = os.cpu_count() or 1
+    n_slots = max(1, min(cfg.R, cores))
+    value, ms = oracle_sample_rate(cfg, n_slots, args.steps, args.warmup, threads=n_slots)
+    sample = f"full MCS (Metropolis+OR+measure+PT) of the first {n_slots} of {cfg.R} temperatures at L={cfg.L}, one thread per replica"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "L": cfg.L, "R": cfg.R, "sampled_replicas": n_slots},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": n_slots, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+    from paper_1211_0780_b200 import binding
+    from paper_1211_0780_b200.build import build_library
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback for the product path)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        build_library()
+    if world > 1:
+        dist.barrier()
+    binding.load_library()
+
+    L, R, N = cfg.L, cfg.R, cfg.L ** 3
+    updates_per_step = 2.0 * N * R
+    xy = binding.XY(L, R, inputs.betas_of(cfg), inputs.SEED + rank)      # independent replica set per rank
+    if cfg.start == "random":
+        xy.init_random()
+    else:
+        xy.init_ordered(0.0)
+    xy.set_option(binding.XY_OPT_PROFILE, 1)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput ("value") ----------------------------------------------------
+    xy.mcs(args.warmup)
+    xy.get_kernel_times()
+    barrier()
+    n0 = xy.get_launch_count()
+    sampler = ClockSampler(local) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.time()
+    e0.record()
+    xy.mcs(args.steps)
+    e1.record()
+    barrier()
+    t1 = time.time()
+    ms_local = e0.elapsed_time(e1)
+    launches = xy.get_launch_count() - n0
+    ktimes = xy.get_kernel_times()
+    clocks = sampler.stop(t0, t1) if sampler else None
+    ms, units = combine_ranks(ms_local, updates_per_step * args.steps, dist if world > 1 else None, "cuda")
+    obs = xy.measure()
+
+    # ---- end to end through the C ABI with HOST buffers ---------------------------------------------
+    # step = xy_set_state(pinned host natural-layout state) -> MCS -> xy_measure(host out) + xy_get_perm(host out)
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    xy.set_option(binding.XY_OPT_PROFILE, 0)
+    host = torch.empty(R * N, dtype=torch.float32, pin_memory=True)
+    xy.get_state(host)
+    for _ in range(2):
+        xy.set_state(host); xy.mcs(1); xy.measure(); xy.get_perm()
+    barrier()
+    e0.record()
+    for _ in range(e2e_steps):
+        xy.set_state(host); xy.mcs(1); xy.measure(); xy.get_perm()
+    e1.record()
+    barrier()
+    e2e_ms, e2e_units = combine_ranks(e0.elapsed_time(e1), updates_per_step * e2e_steps, dist if world > 1 else None, "cuda")
+
+    if world > 1:
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+    peak, peak_src = measured_peak_gbs()
+    # dominant kernel = the class with the largest device time in the timed region
+    dom = max(("metropolis", "overrelax", "measure"), key=lambda k: ktimes[k][0])
+    per_launch_bytes = {"metropolis": BYTES_PER_UPDATE * N * R / 2, "overrelax": BYTES_PER_UPDATE * N * R / 2,
+                        "measure": 4.0 * N * R}
+    kern = {}
+    for k, (tot, n) in ktimes.items():
+        if n:
+            kern[k] = {"launches": n, "avg_ms": tot / n, "share": tot / (ms_local + 1e-30)}
+            if k in per_launch_bytes:
+                kern[k]["algorithmic_GBps"] = per_launch_bytes[k] / (tot / n * 1e-3) * 1e-9
+    ach = kern[dom]["algorithmic_GBps"]
+    traffic = NCU_TRAFFIC_BYTES.get(cfg.name, {}).get(dom)
+    out = {
+        "metric": METRIC, "value": units / (ms * 1e-3) * 1e-9, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": cfg.name, "L": L, "R": R, "beta": [cfg.beta_lo, cfg.beta_hi], "start": cfg.start,
+                   "state_bytes": 4 * N * R, "l2": "inputs larger than L2 (state 1.05 GB >> 126 MB)" if 4 * N * R > 4e8
+                   else "state fits in L2; no flush", "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "tile_y": xy.get_option(binding.XY_OPT_TILE_Y), "tile_z": xy.get_option(binding.XY_OPT_TILE_Z)},
+        "site_mcs_per_ns": units / 2 / (ms * 1e-3) * 1e-9,
+        "hbm_roofline_frac_whole_mcs": units * BYTES_PER_UPDATE / (ms * 1e-3) * 1e-9 / peak,
+        "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
+                     "frac": ach / peak, "traffic": traffic, "bytes_per_update": BYTES_PER_UPDATE,
+                     "algorithmic_bytes_per_launch": per_launch_bytes[dom]},
+        "kernels": kern,
+        "e2e": {"value": e2e_units / (e2e_ms * 1e-3) * 1e-9, "unit": UNIT, "h2d_bytes_per_step": 4 * N * R,
+                "d2h_bytes_per_step": R * 5 * 8 + R * 4, "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps,
+                "call": "xy_set_state(pinned host) -> xy_mcs(1) -> xy_measure(host) + xy_get_perm(host)"},
+        "gpu_launches": launches,
+        "clocks": clocks,
+        "observables_rank0": {"E_per_site": obs[0, 0] / N, "m": float(np.sqrt(obs[0, 3])) / N},
+    }
+    if not args.no_cpu_baseline and world == 1:
+        cores = os.cpu_count() or 1
+        n_slots = max(1, min(R, cores))
+        v, _ = oracle_sample_rate(cfg, n_slots, 2, 1, threads=n_slots)
+        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": n_slots, "kind": "oracle",
+                               "sample": f"2 timed MCS (after 1 warm-up) of the first {n_slots} of {R} temperatures at L={L}, "
+                                         "one thread per replica"}
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="index into BASELINE.json configs (default 4: L=160, R=64)")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    cfg = inputs.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

@@ -52,8 +52,21 @@ enum {
     XY_OPT_TILE_Z = 2,     /* planes a thread block marches through (must divide L)                  */
     XY_OPT_TRACE = 3,      /* 1: xy_metropolis_sweep also records its fast-path acceptance probability
                               per site (test hook; allocates R*N floats inside the library)         */
-    XY_OPT_FUSED_MEASURE = 4 /* 1 (default): the white over-relaxation pass also accumulates the
+    XY_OPT_FUSED_MEASURE = 4, /* 1: the white over-relaxation pass also accumulates the
                               observables, so xy_measure after xy_overrelax_sweep reads no spins    */
+    XY_OPT_PROFILE = 5     /* 1: bracket every kernel launch with a CUDA-event pair on the attached
+                              stream; xy_get_kernel_times returns the per-class device times         */
+};
+
+/* Kernel classes reported by xy_get_kernel_times. */
+#define XY_NUM_KERNEL_CLASSES 6
+enum {
+    XY_K_METROPOLIS = 0, /* one Metropolis colour pass over all slots (a2)                         */
+    XY_K_OVERRELAX = 1,  /* one over-relaxation colour pass over all slots (a3)                    */
+    XY_K_MEASURE = 2,    /* the observable reduction over all slots (a4, first stage)              */
+    XY_K_FINALIZE = 3,   /* a4 final stage: per-slot sums in fixed order, by-rank output           */
+    XY_K_PT = 4,         /* the replica-exchange kernel (a5)                                       */
+    XY_K_OTHER = 5       /* init, fill, layout conversion                                          */
 };
 
 /* ---- lifetime ------------------------------------------------------------------------------ */
@@ -155,6 +168,10 @@ int xy_set_option(xy_ctx* ctx, int option, int value);
 int xy_get_option(xy_ctx* ctx, int option, int* value);
 /* Number of kernels this context has launched since attach (bench.py's gpu_launches). */
 int xy_get_launch_count(xy_ctx* ctx, uint64_t* n);
+/* With XY_OPT_PROFILE = 1: device time in milliseconds (CUDA events on the attached stream) and
+ * number of launches per kernel class since the previous call; ms and launches have
+ * XY_NUM_KERNEL_CLASSES entries.  Synchronises, then resets the accumulators. */
+int xy_get_kernel_times(xy_ctx* ctx, double* ms, uint64_t* launches);
 int xy_synchronize(xy_ctx* ctx);
 const char* xy_last_error(void);
 

@@ -77,12 +77,41 @@ struct xy_ctx {
     // cache state
     bool partials_valid = false, rank_valid = false;
     uint64_t launches = 0;
+    // XY_OPT_PROFILE: one CUDA-event pair around every launch, resolved by xy_get_kernel_times
+    int profile = 0;
+    struct Span { cudaEvent_t a, b; int cls; };
+    std::vector<Span> spans;
+    std::vector<cudaEvent_t> free_events;
+    double k_ms[XY_NUM_KERNEL_CLASSES] = {};
+    uint64_t k_n[XY_NUM_KERNEL_CLASSES] = {};
 
     float* colour(int c) const { return d_state + (size_t)c * R * half_n; }
     template <class T> T* ws_ptr(size_t off) const { return reinterpret_cast<T*>(d_ws + off); }
 };
 
 namespace {
+
+// Brackets one kernel launch with a pair of events on the context's stream when profiling is on.
+struct LaunchSpan {
+    xy_ctx* c; int cls; cudaEvent_t a = nullptr, b = nullptr;
+    static cudaEvent_t take(xy_ctx* c) {
+        cudaEvent_t e = nullptr;
+        if (!c->free_events.empty()) { e = c->free_events.back(); c->free_events.pop_back(); }
+        else if (cudaEventCreate(&e) != cudaSuccess) e = nullptr;
+        return e;
+    }
+    LaunchSpan(xy_ctx* ctx, int k) : c(ctx), cls(k) {
+        ++c->launches;
+        if (!c->profile) return;
+        a = take(c); b = take(c);
+        if (a) cudaEventRecord(a, c->stream);
+    }
+    ~LaunchSpan() {
+        if (!c->profile || !a || !b) return;
+        cudaEventRecord(b, c->stream);
+        c->spans.push_back({a, b, cls});
+    }
+};
 
 void default_tiles(int L, int R, int& TY, int& TZ) {
     const int W4 = L / 8;
@@ -116,9 +145,11 @@ int launch_sweep(xy_ctx* c, const SweepParams& P) {
     int threads = P.nItems > 2 * P.W4 ? P.nItems : 2 * P.W4;
     threads = (threads + 31) / 32 * 32;
     dim3 grid(P.nTY * P.nTZ, c->R);
-    sweep_kernel<MODE, TRACE><<<grid, threads, smem, c->stream>>>(P);
+    {
+        LaunchSpan span(c, MODE == MODE_MET ? XY_K_METROPOLIS : MODE == MODE_OR ? XY_K_OVERRELAX : XY_K_MEASURE);
+        sweep_kernel<MODE, TRACE><<<grid, threads, smem, c->stream>>>(P);
+    }
     CK(cudaGetLastError());
-    ++c->launches;
     return XY_OK;
 }
 
@@ -177,12 +208,14 @@ int run_measure(xy_ctx* c, double* d_series_row) {
     }
     if (!c->rank_valid || d_series_row) {
         const int n_tiles = (c->L / c->TY) * (c->L / c->TZ);
-        measure_finalize_kernel<<<c->R, 128, 0, c->stream>>>(c->ws_ptr<double>(c->ws.partials), n_tiles,
-                                                             c->ws_ptr<int>(c->ws.slot_at_rank),
-                                                             c->ws_ptr<double>(c->ws.obs_rank),
-                                                             c->ws_ptr<double>(c->ws.obs_slot), d_series_row);
+        {
+            LaunchSpan span(c, XY_K_FINALIZE);
+            measure_finalize_kernel<<<c->R, 128, 0, c->stream>>>(c->ws_ptr<double>(c->ws.partials), n_tiles,
+                                                                 c->ws_ptr<int>(c->ws.slot_at_rank),
+                                                                 c->ws_ptr<double>(c->ws.obs_rank),
+                                                                 c->ws_ptr<double>(c->ws.obs_slot), d_series_row);
+        }
         CK(cudaGetLastError());
-        ++c->launches;
         c->rank_valid = true;
     }
     return XY_OK;
@@ -213,6 +246,8 @@ void xy_destroy(xy_ctx* c) {
     if (c->own_state && c->d_state) cudaFree(c->d_state);
     if (c->own_ws && c->d_ws) cudaFree(c->d_ws);
     if (c->d_trace) cudaFree(c->d_trace);
+    for (auto& s : c->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
+    for (auto e : c->free_events) cudaEventDestroy(e);
     delete c;
 }
 
@@ -248,9 +283,11 @@ int xy_attach(xy_ctx* c, void* d_state, void* d_workspace, void* cuda_stream) {
 int xy_init_random(xy_ctx* c) {
     if (int rc = need(c)) return rc;
     const size_t n_quads = (size_t)c->R * c->L * c->L * (c->L / 4);
-    init_random_kernel<<<grid_for(n_quads, 256), 256, 0, c->stream>>>(c->colour(0), c->colour(1), c->L, c->R, c->keys);
+    {
+        LaunchSpan span(c, XY_K_OTHER);
+        init_random_kernel<<<grid_for(n_quads, 256), 256, 0, c->stream>>>(c->colour(0), c->colour(1), c->L, c->R, c->keys);
+    }
     CK(cudaGetLastError());
-    ++c->launches;
     c->partials_valid = false;
     return XY_OK;
 }
@@ -258,9 +295,11 @@ int xy_init_random(xy_ctx* c) {
 int xy_init_ordered(xy_ctx* c, float theta0) {
     if (int rc = need(c)) return rc;
     const size_t n = (size_t)c->R * c->N;
-    fill_kernel<<<grid_for(n, 256), 256, 0, c->stream>>>(c->d_state, n, theta0);
+    {
+        LaunchSpan span(c, XY_K_OTHER);
+        fill_kernel<<<grid_for(n, 256), 256, 0, c->stream>>>(c->d_state, n, theta0);
+    }
     CK(cudaGetLastError());
-    ++c->launches;
     c->partials_valid = false;
     return XY_OK;
 }
@@ -270,15 +309,16 @@ static int convert_state(xy_ctx* c, float* black, float* white, float* natural, 
     const size_t per_slot = (size_t)L * L * (L / 8);
     if (on_device) {
         const size_t n = per_slot * c->R;
+        LaunchSpan span(c, XY_K_OTHER);
         if (to_split) convert_kernel<true><<<grid_for(n, 256), 256, 0, c->stream>>>(natural, black, white, L, c->R, 0);
         else convert_kernel<false><<<grid_for(n, 256), 256, 0, c->stream>>>(natural, black, white, L, c->R, 0);
         CK(cudaGetLastError());
-        ++c->launches;
         return XY_OK;
     }
     float* stage = c->ws_ptr<float>(c->ws.stage);
     for (int r = 0; r < c->R; ++r) {            // one natural slot at a time through the staging buffer
         float* h = natural + (size_t)r * c->N;
+        LaunchSpan span(c, XY_K_OTHER);
         if (to_split) {
             CK(cudaMemcpyAsync(stage, h, c->N * 4, cudaMemcpyHostToDevice, c->stream));
             convert_kernel<true><<<grid_for(per_slot, 256), 256, 0, c->stream>>>(stage, black, white, L, 1, r);
@@ -287,7 +327,6 @@ static int convert_state(xy_ctx* c, float* black, float* white, float* natural, 
             CK(cudaMemcpyAsync(h, stage, c->N * 4, cudaMemcpyDeviceToHost, c->stream));
         }
         CK(cudaGetLastError());
-        ++c->launches;
     }
     CK(cudaStreamSynchronize(c->stream));
     return XY_OK;
@@ -347,12 +386,14 @@ int xy_pt_exchange(xy_ctx* c) {
     if (int rc = need(c)) return rc;
     if (int rc = run_measure(c, nullptr)) return rc;
     const int pairs = c->R / 2 + 1;
-    pt_exchange_kernel<<<(pairs + 127) / 128, 128, 0, c->stream>>>(
-        c->R, c->n_pt, c->keys, c->ws_ptr<double>(c->ws.betas), c->ws_ptr<double>(c->ws.obs_slot),
-        c->ws_ptr<int>(c->ws.slot_at_rank), c->ws_ptr<double>(c->ws.beta_of_slot), c->ws_ptr<float>(c->ws.beta32),
-        c->ws_ptr<unsigned long long>(c->ws.pt_acc));
+    {
+        LaunchSpan span(c, XY_K_PT);
+        pt_exchange_kernel<<<(pairs + 127) / 128, 128, 0, c->stream>>>(
+            c->R, c->n_pt, c->keys, c->ws_ptr<double>(c->ws.betas), c->ws_ptr<double>(c->ws.obs_slot),
+            c->ws_ptr<int>(c->ws.slot_at_rank), c->ws_ptr<double>(c->ws.beta_of_slot), c->ws_ptr<float>(c->ws.beta32),
+            c->ws_ptr<unsigned long long>(c->ws.pt_acc));
+    }
     CK(cudaGetLastError());
-    ++c->launches;
     ++c->n_pt;
     c->rank_valid = false;
     return XY_OK;
@@ -436,6 +477,7 @@ int xy_set_option(xy_ctx* c, int option, int value) {
             c->TZ = value; c->partials_valid = false; return XY_OK;
         case XY_OPT_TRACE: c->trace = value ? 1 : 0; return XY_OK;
         case XY_OPT_FUSED_MEASURE: c->fused = value ? 1 : 0; return XY_OK;
+        case XY_OPT_PROFILE: c->profile = value ? 1 : 0; return XY_OK;
         default: return fail(XY_ERR_INVALID_ARG, "unknown option %d", option);
     }
 }
@@ -447,8 +489,26 @@ int xy_get_option(xy_ctx* c, int option, int* value) {
         case XY_OPT_TILE_Z: *value = c->TZ; return XY_OK;
         case XY_OPT_TRACE: *value = c->trace; return XY_OK;
         case XY_OPT_FUSED_MEASURE: *value = c->fused; return XY_OK;
+        case XY_OPT_PROFILE: *value = c->profile; return XY_OK;
         default: return fail(XY_ERR_INVALID_ARG, "unknown option %d", option);
     }
+}
+
+int xy_get_kernel_times(xy_ctx* c, double* ms, uint64_t* n) {
+    if (int rc = need(c)) return rc;
+    if (!ms || !n) return fail(XY_ERR_INVALID_ARG, "xy_get_kernel_times: NULL pointer");
+    CK(cudaStreamSynchronize(c->stream));
+    for (auto& s : c->spans) {
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, s.a, s.b));
+        c->k_ms[s.cls] += (double)t;
+        c->k_n[s.cls] += 1;
+        c->free_events.push_back(s.a);
+        c->free_events.push_back(s.b);
+    }
+    c->spans.clear();
+    for (int k = 0; k < XY_NUM_KERNEL_CLASSES; ++k) { ms[k] = c->k_ms[k]; n[k] = c->k_n[k]; c->k_ms[k] = 0.0; c->k_n[k] = 0; }
+    return XY_OK;
 }
 
 int xy_get_launch_count(xy_ctx* c, uint64_t* n) {

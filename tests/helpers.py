@@ -52,13 +52,13 @@ def predicted_init(L, R, seed):
     return out
 
 
-def predicted_proposals(L, R, n_met, seed):
-    """(theta_new, u) every site would draw in Metropolis sweep number n_met."""
+def predicted_proposals(L, R, n_met, seed, slots=None):
+    """(theta_new, u) every site would draw in Metropolis sweep number n_met (only `slots` filled if given)."""
     z, y, x = np.meshgrid(np.arange(L), np.arange(L), np.arange(L), indexing="ij")
     colour = (x + y + z) & 1
     prop = np.empty((R, L, L, L), dtype=np.float32)
     uacc = np.empty((R, L, L, L), dtype=np.float32)
-    for r in range(R):
+    for r in (range(R) if slots is None else slots):
         Wb, i = site_words(L, r, n_met, STREAM_MET_BLACK, seed)
         Ww, _ = site_words(L, r, n_met, STREAM_MET_WHITE, seed)
         W = np.where(colour[None] == 0, Wb, Ww)

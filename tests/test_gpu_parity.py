@@ -1,0 +1,477 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Protocol: the MCS map is chaotic, so every comparison is
+LOCK-STEP -- both sides start one call from the same state and counters.  A sweep is two colour
+passes; the oracle is run pass by pass from exactly the neighbourhood the GPU saw (the white
+pass from the GPU's own black result), so each decision / reflection is compared like for like.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_1211_0780_b200 import inputs
+from . import helpers as H
+from . import parity as P
+
+pytestmark = pytest.mark.gpu
+SEED = inputs.SEED
+NCPU = max(1, min(32, os.cpu_count() or 1))
+
+# (L, R): several tiles in y and z, ragged row lengths (L/8 = 1, 3, 5 float4 per row), R = 1
+SHAPES = [(8, 8), (16, 3), (24, 5), (32, 16), (40, 2), (48, 1), (64, 4)]
+
+
+def make(xy_mod, oracle_mod, L, R, betas=None, seed=SEED):
+    betas = inputs.beta_ladder(0.44, 0.47, R) if betas is None else np.asarray(betas, dtype=np.float64)
+    xy = xy_mod.XY(L, R, betas, seed)
+    ora = oracle_mod.XYOracle(L, R, betas, seed, threads=NCPU)
+    return xy, ora
+
+
+def states_for(L, R):
+    yield "uniform", inputs.uniform_state(L, R, 11)
+    yield "smooth", inputs.smooth_state(L, R, 12)
+
+
+def metropolis_lockstep(xy, ora, S, t, slots=None):
+    """One GPU Metropolis sweep from state S with n_met = t, checked pass by pass (P1)."""
+    L, R = xy.L, xy.R
+    col = H.colour_mask(L)
+    xy.set_state(S); xy.set_counters([t, 0, 0])
+    perm = xy.get_perm()
+    xy.metropolis_sweep()
+    G = xy.get_state()
+    prop, _ = H.predicted_proposals(L, R, t, SEED, slots)
+    ora.set_perm(perm); ora.set_counters([t, 0, 0]); ora.set_active_slots(slots)
+    out = []
+    start = S
+    for c in (0, 1):
+        sel = np.zeros((R, L, L, L), dtype=bool)
+        sel[list(range(R)) if slots is None else list(slots)] = (col == c)
+        ora.set_state(start)
+        tr = ora.enable_trace(met=True)
+        ora.metropolis_pass(c)
+        out.append(P.check_metropolis(start, G, ora.get_state(), prop, tr["met_p"], tr["met_u"], sel))
+        start = np.where(col[None] == 0, G, S)          # the GPU's black result + the untouched white sites
+    ora.enable_trace()
+    # untouched sites of other slots / nothing else changed
+    assert np.array_equal(xy.get_counters(), [t + 1, 0, 0])
+    return out
+
+
+def overrelax_lockstep(xy, ora, S, slots=None):
+    L, R = xy.L, xy.R
+    col = H.colour_mask(L)
+    xy.set_state(S)
+    xy.overrelax_sweep()
+    G = xy.get_state()
+    ora.set_active_slots(slots)
+    out = []
+    start = S
+    for c in (0, 1):
+        sel = np.zeros((R, L, L, L), dtype=bool)
+        sel[list(range(R)) if slots is None else list(slots)] = (col == c)
+        ora.set_state(start)
+        tr = ora.enable_trace(overrelax=True)
+        ora.overrelax_pass(c)
+        out.append(P.check_overrelax(G, ora.get_state(), tr["or_h"], sel))
+        start = np.where(col[None] == 0, G, S)
+    ora.enable_trace()
+    return out, G
+
+
+# ---- a1 / device math -------------------------------------------------------------------------
+def test_device_philox_known_answers_and_random_counters(xy_mod):
+    kat = []
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "philox4x32_10_kat.txt")):
+        line = line.split("#")[0].split()
+        if len(line) == 10:
+            kat.append([int(v, 16) for v in line])
+    assert len(kat) >= 3
+    for row in kat:
+        out = xy_mod.debug_philox(np.array([row[0:4]], dtype=np.uint32), row[4], row[5])
+        assert [int(v) for v in out[0]] == row[6:10]
+    rng = np.random.default_rng(5)
+    ctr = rng.integers(0, 2 ** 32, size=(4096, 4), dtype=np.uint64).astype(np.uint32)
+    k0, k1 = 0x12110780, 0xDEADBEEF
+    out = xy_mod.debug_philox(ctr, k0, k1)
+    ref = np.stack(H.philox4x32_10_np(ctr[:, 0], ctr[:, 1], ctr[:, 2], ctr[:, 3], k0, k1), axis=1)
+    assert np.array_equal(out, ref)
+
+
+def test_device_math_errors(xy_mod):
+    """The stated errors of the kernels' fast math (parity.EPS_SINCOS and DESIGN.md section 6)."""
+    rng = np.random.default_rng(6)
+    x = np.concatenate([rng.random(1 << 20) * 2 * np.pi, [0.0, np.pi / 2, np.pi, 3 * np.pi / 2, 6.2831855],
+                        (np.arange(1 << 16) * (2 * np.pi / (1 << 16)))]).astype(np.float32)
+    c, s = xy_mod.debug_sincos(x)
+    ec = c.astype(np.float64) - np.cos(x.astype(np.float64))
+    es = s.astype(np.float64) - np.sin(x.astype(np.float64))
+    print(f"sincos: max|err| cos {np.abs(ec).max():.3e} sin {np.abs(es).max():.3e}; bias cos {ec.mean():.2e} sin {es.mean():.2e};"
+          f" rms {np.sqrt((ec ** 2).mean()):.2e}")
+    assert np.abs(ec).max() <= P.EPS_SINCOS and np.abs(es).max() <= P.EPS_SINCOS
+    assert abs(ec.mean()) < 2e-8 and abs(es.mean()) < 2e-8
+    phi = rng.random(1 << 20) * 2 * np.pi
+    r = np.exp(rng.uniform(np.log(1e-6), np.log(6.0), size=phi.size))
+    hx, hy = (r * np.cos(phi)).astype(np.float32), (r * np.sin(phi)).astype(np.float32)
+    a = xy_mod.debug_atan2(hy, hx)
+    ref = np.arctan2(hy.astype(np.float64), hx.astype(np.float64)) % (2 * np.pi)
+    ea = H.angle_diff(a, ref)
+    print(f"atan2: max|err| {ea.max():.3e}")
+    assert ea.max() <= 6e-7
+    assert a.min() >= 0.0 and a.max() <= 6.2831855
+    for yy, xx, want in ((0.0, 1.0, 0.0), (1.0, 0.0, np.pi / 2), (0.0, -1.0, np.pi), (-1.0, 0.0, 3 * np.pi / 2),
+                         (1.0, 1.0, np.pi / 4), (-1.0, -1.0, 5 * np.pi / 4)):
+        got = xy_mod.debug_atan2(np.array([yy]), np.array([xx]))[0]
+        assert abs(got - want) <= 6e-7
+
+
+# ---- a0 -------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L,R", [(8, 8), (24, 3), (32, 4)])
+def test_init_random_is_bit_exact(xy_mod, oracle_mod, L, R):
+    xy, ora = make(xy_mod, oracle_mod, L, R)
+    xy.init_random(); ora.init_random()
+    G = xy.get_state()
+    assert np.array_equal(G.view(np.uint32), H.predicted_init(L, R, SEED).view(np.uint32))
+    assert np.array_equal(G.view(np.uint32), ora.get_state().view(np.uint32))
+    xy.init_ordered(0.25)
+    assert np.all(xy.get_state() == np.float32(0.25))
+
+
+@pytest.mark.parametrize("L,R", [(8, 2), (40, 3)])
+def test_state_roundtrip_host_and_device(xy_mod, L, R):
+    import torch
+    xy = xy_mod.XY(L, R, inputs.beta_ladder(0.4, 0.5, R), SEED)
+    S = inputs.uniform_state(L, R, 3)
+    xy.set_state(S)
+    assert np.array_equal(xy.get_state().view(np.uint32), S.view(np.uint32))
+    d = torch.from_numpy(S).cuda()
+    xy.init_ordered(0.0)
+    xy.set_state(d)
+    out = torch.empty_like(d)
+    xy.get_state(out)
+    assert torch.equal(out, d)
+
+
+# ---- a2 -------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L,R", SHAPES)
+def test_metropolis_lockstep(xy_mod, oracle_mod, L, R):
+    xy, ora = make(xy_mod, oracle_mod, L, R)
+    for name, S in states_for(L, R):
+        for t in (0, 7):
+            stats = metropolis_lockstep(xy, ora, S, t)
+            print(L, R, name, t, stats)
+            assert 0.2 < stats[0]["accept_frac"] < 0.95
+    met, _ = xy.get_accept_counts()
+    assert met.sum() > 0
+
+
+def test_metropolis_other_tilings_give_identical_states(xy_mod):
+    """The tiling is an implementation detail: any valid (TILE_Y, TILE_Z) gives the same bits."""
+    L, R = 32, 3
+    S = inputs.uniform_state(L, R, 21)
+    ref = None
+    for ty, tz in ((32, 32), (8, 8), (16, 4), (4, 2), (2, 16)):
+        xy = xy_mod.XY(L, R, inputs.beta_ladder(0.45, 0.46, R), SEED)
+        xy.set_option(xy_mod.XY_OPT_TILE_Z, tz); xy.set_option(xy_mod.XY_OPT_TILE_Y, ty)
+        xy.set_state(S); xy.metropolis_sweep(); xy.overrelax_sweep()
+        G = xy.get_state()
+        obs = xy.measure()
+        if ref is None:
+            ref, ref_obs = G, obs
+        assert np.array_equal(G.view(np.uint32), ref.view(np.uint32)), (ty, tz)
+        assert np.allclose(obs, ref_obs, rtol=1e-9, atol=1e-6)
+
+
+def test_metropolis_extreme_betas(xy_mod, oracle_mod):
+    """beta = 0 accepts everything (state predictable from Philox alone, O1); beta huge and an
+    ordered start accepts nothing (O3); negative beta is legal (antiferromagnet)."""
+    L, R = 16, 4
+    xy, ora = make(xy_mod, oracle_mod, L, R, betas=[0.0, 1e30, -0.3, 0.0])
+    S = inputs.ordered_state(L, R)
+    xy.set_state(S); xy.set_counters([3, 0, 0]); xy.metropolis_sweep()
+    G = xy.get_state()
+    prop, _ = H.predicted_proposals(L, R, 3, SEED)
+    for r in (0, 3):
+        assert np.array_equal(G[r].view(np.uint32), prop[r].view(np.uint32))
+    assert np.all(G[1] == 0.0)
+    metropolis_lockstep(xy, ora, inputs.uniform_state(L, R, 4), 1)
+
+
+# ---- a3 -------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L,R", SHAPES)
+def test_overrelax_lockstep(xy_mod, oracle_mod, L, R):
+    xy, ora = make(xy_mod, oracle_mod, L, R)
+    for name, S in states_for(L, R):
+        xy.set_state(S)
+        E0 = xy.measure()[:, 0]
+        stats, G = overrelax_lockstep(xy, ora, S)
+        print(L, R, name, stats)
+        assert np.all((G >= 0.0) & (G <= np.float32(6.2831855)))
+        E1 = xy.measure()[:, 0]
+        assert np.all(np.abs(E1 - E0) <= 1e-5 * np.abs(E0) + 1e-3), "over-relaxation must conserve E (P:43)"
+    assert np.array_equal(xy.get_counters(), [0, 2, 0])
+
+
+def test_overrelax_fixed_points_and_vanishing_field(xy_mod, oracle_mod):
+    """Helical states are fixed points (h_i parallel to S_i, O7).  Where the field (nearly)
+    vanishes the reflection is ill-conditioned: the result must stay a finite angle in range and
+    pass the conditioned clause of P2 (R6: h = 0 exactly leaves the spin alone)."""
+    L, R = 16, 2
+    xy, ora = make(xy_mod, oracle_mod, L, R, betas=[0.45, 0.46])
+    for k in ((1, 0, 0), (0, 2, 0), (0, 0, 3), (1, 1, 1)):
+        S = inputs.helical_state(L, R, k, phase=0.3)
+        xy.set_state(S); xy.overrelax_sweep()
+        assert H.angle_diff(xy.get_state(), S).max() < 5e-6
+    # 2x2x2 blocks of 0 / pi: every site sees three neighbours at 0 and three at pi -> |h| ~ 1e-7
+    z, y, x = np.meshgrid(np.arange(L), np.arange(L), np.arange(L), indexing="ij")
+    S = np.where((x // 2 + y // 2 + z // 2) % 2 == 0, 0.0, np.pi).astype(np.float32)
+    S = np.broadcast_to(S, (R, L, L, L)).copy()
+    stats, G = overrelax_lockstep(xy, ora, S)
+    assert np.isfinite(G).all() and G.min() >= 0.0 and G.max() <= np.float32(6.2831855)
+
+
+# ---- a4 -------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L,R", SHAPES)
+def test_measure_against_oracle(xy_mod, oracle_mod, L, R):
+    xy, ora = make(xy_mod, oracle_mod, L, R)
+    for name, S in states_for(L, R):
+        xy.set_state(S); ora.set_state(S)
+        stats = P.check_observables(xy.measure(), ora.measure(), L ** 3)
+        print(L, R, name, stats)
+    # by RANK: after a permutation the rows move with the labels
+    if R >= 3:
+        perm = np.roll(np.arange(R, dtype=np.int32), 1)
+        xy.set_perm(perm); ora.set_perm(perm)
+        g = xy.measure()
+        P.check_observables(g, ora.measure(), L ** 3)
+        assert np.array_equal(xy.get_perm(), perm)
+        assert np.allclose(xy.get_beta_of_slot()[perm], inputs.beta_ladder(0.44, 0.47, R))
+
+
+def test_measure_closed_forms(xy_mod):
+    """O3 / O7 / O8 on the GPU reduction: ordered, helical (each axis separately) and staggered."""
+    L, R = 16, 2
+    N = L ** 3
+    xy = xy_mod.XY(L, R, [0.45, 0.46], SEED)
+    xy.set_state(inputs.ordered_state(L, R, 0.0))
+    o = xy.measure()
+    assert np.allclose(o, [[-3.0 * N, N, 0.0, float(N) ** 2, float(N) ** 4]] * R, rtol=1e-7, atol=1e-3)
+    for k in ((1, 0, 0), (0, 2, 0), (0, 0, 3), (2, 1, 3)):
+        xy.set_state(inputs.helical_state(L, R, k))
+        o = xy.measure()
+        E = -N * sum(np.cos(2 * np.pi * kk / L) for kk in k)
+        assert np.all(np.abs(o[:, 0] - E) <= 1e-6 * 3 * N), (k, o[:, 0], E)
+        assert np.all(np.abs(o[:, 1:3]) <= 1e-6 * N)
+    xy.set_state(inputs.staggered_state(L, R))
+    o = xy.measure()
+    assert np.all(np.abs(o[:, 0] - 3.0 * N) <= 1e-6 * 3 * N) and np.all(np.abs(o[:, 1:3]) <= 1e-6 * N)
+    # global rotation leaves E and |M|^2 unchanged (O6)
+    S = inputs.smooth_state(L, R, 9)
+    xy.set_state(S); a = xy.measure()
+    xy.set_state(((S.astype(np.float64) + 1.2345) % (2 * np.pi)).astype(np.float32)); b = xy.measure()
+    assert np.all(np.abs(a[:, 0] - b[:, 0]) <= 2e-6 * 3 * N)
+    assert np.allclose(a[:, 3], b[:, 3], rtol=1e-5)
+
+
+def test_measure_is_deterministic_and_cached(xy_mod):
+    L, R = 32, 4
+    xy = xy_mod.XY(L, R, inputs.beta_ladder(0.45, 0.46, R), SEED)
+    xy.init_random()
+    a = xy.measure()
+    n0 = xy.get_launch_count()
+    b = xy.measure()
+    assert xy.get_launch_count() == n0, "an unchanged state must not be reduced again"
+    assert np.array_equal(a, b)
+    xy.set_state(xy.get_state())
+    assert np.array_equal(xy.measure(), a), "fixed-order reduction: bit-identical run to run"
+
+
+# ---- a5 -------------------------------------------------------------------------------------
+def test_pt_forced_swaps_at_equal_beta(xy_mod):
+    """O10: all beta equal -> every attempted pair swaps; the permutation after t exchanges is known."""
+    for R in (1, 2, 5, 8):
+        xy = xy_mod.XY(8, R, [0.45] * R, SEED)
+        xy.init_random()
+        want = list(range(R))
+        for t in range(6):
+            xy.pt_exchange()
+            for k in range(t & 1, R - 1, 2):
+                want[k], want[k + 1] = want[k + 1], want[k]
+            assert list(xy.get_perm()) == want
+        assert np.array_equal(xy.get_counters(), [0, 0, 6])
+        _, pt = xy.get_accept_counts()
+        assert pt.sum() == sum(len(range(t & 1, R - 1, 2)) for t in range(6))
+
+
+@pytest.mark.parametrize("L,R,lo,hi", [(8, 8, 0.44, 0.47), (16, 16, 0.40, 0.50), (32, 16, 0.450, 0.458)])
+def test_pt_lockstep(xy_mod, oracle_mod, L, R, lo, hi):
+    """P4: both sides compute E from the shared state; decisions and label bookkeeping agree."""
+    betas = inputs.beta_ladder(lo, hi, R)
+    xy, ora = make(xy_mod, oracle_mod, L, R, betas=betas)
+    # replicas thermalised a little so that energies are ordered like the betas
+    xy.init_random()
+    xy.mcs(30)
+    n_swapped = 0
+    for t in range(30, 50):
+        S, perm = xy.get_state(), xy.get_perm()
+        ora.set_state(S); ora.set_perm(perm); ora.set_counters([0, 0, t])
+        xy.set_counters([0, 0, t])
+        tr = ora.enable_trace(pt=True)
+        xy.pt_exchange(); ora.pt_exchange()
+        g = xy.get_perm()
+        P.check_pt(g, ora.get_perm(), tr["pt_p"], tr["pt_u"])
+        n_swapped += int((g != perm).sum()) // 2
+        bos = xy.get_beta_of_slot()
+        assert np.array_equal(bos[g], betas), "beta labels must follow slot_at_rank"
+        assert np.array_equal(bos, ora.get_beta_of_slot()) or not np.array_equal(g, ora.get_perm())
+        xy.metropolis_sweep(); xy.overrelax_sweep()
+    assert n_swapped > 0
+
+
+# ---- one full MCS (P5) and free run (P6) --------------------------------------------------------
+def mcs_lockstep(xy, ora, t):
+    """Advance the GPU one MCS from its current state with counters (t,t,t); check every stage."""
+    L, R = xy.L, xy.R
+    S, perm = xy.get_state(), xy.get_perm()
+    metropolis_lockstep(xy, ora, S, t)
+    S1 = xy.get_state()
+    _, S2 = overrelax_lockstep(xy, ora, S1)
+    ora.set_state(S2); ora.set_perm(perm); ora.set_counters([t + 1, t + 1, t])
+    xy.set_counters([t + 1, t + 1, t])
+    obs = xy.measure()
+    P.check_observables(obs, ora.measure(), L ** 3)
+    tr = ora.enable_trace(pt=True)
+    xy.pt_exchange(); ora.pt_exchange()
+    P.check_pt(xy.get_perm(), ora.get_perm(), tr["pt_p"], tr["pt_u"])
+    ora.enable_trace()
+    return obs
+
+
+@pytest.mark.parametrize("idx,n_mcs", [(0, 200), (1, 60), (2, 12)])
+def test_full_mcs_lockstep_on_configs(xy_mod, oracle_mod, idx, n_mcs):
+    """P5 on BASELINE.json configs 1-3: a free-running GPU trajectory, every sampled MCS re-done
+    by the oracle from the GPU's state."""
+    cfg = inputs.CONFIGS[idx]
+    xy, ora = make(xy_mod, oracle_mod, cfg.L, cfg.R, betas=inputs.betas_of(cfg))
+    xy.init_random()
+    sampled = sorted(set(list(range(min(10, n_mcs))) + [n_mcs // 4, n_mcs // 2, n_mcs - 1]))
+    t = 0
+    for s in sampled:
+        if s > t:
+            xy.mcs(s - t)
+            t = s
+        assert np.array_equal(xy.get_counters(), [t, t, t])
+        mcs_lockstep(xy, ora, t)
+        t += 1
+
+
+def test_free_run_divergence_report(xy_mod, oracle_mod):
+    """P6: GPU and oracle run freely from the same start.  Only k = 1 is asserted (chaos: the
+    difference grows x3-5 per MCS, SURVEY.md finding 3); the curve is printed."""
+    L, R = 16, 4
+    xy, ora = make(xy_mod, oracle_mod, L, R, betas=inputs.beta_ladder(0.45, 0.458, R))
+    xy.init_random(); ora.init_random()
+    curve = []
+    for k in range(1, 13):
+        xy.mcs(1); ora.mcs()
+        d = H.angle_diff(xy.get_state(), ora.get_state())
+        curve.append((k, float(np.sqrt((d ** 2).mean())), float(d.max())))
+    print("free-run rms/max difference per MCS:", curve)
+    assert curve[0][2] <= 1e-3 and curve[0][1] <= 1e-5
+
+
+def test_mcs_series_matches_stepwise_calls(xy_mod):
+    """xy_mcs(n) with a device series == n x (sweep, sweep, measure, exchange) called one by one."""
+    import torch
+    L, R, n = 16, 6, 9
+    betas = inputs.beta_ladder(0.44, 0.47, R)
+    a = xy_mod.XY(L, R, betas, SEED); b = xy_mod.XY(L, R, betas, SEED)
+    a.init_random(); b.init_random()
+    series = torch.zeros(n, R, 5, dtype=torch.float64, device="cuda")
+    a.mcs(n, series)
+    rows = []
+    for _ in range(n):
+        b.metropolis_sweep(); b.overrelax_sweep(); rows.append(b.measure()); b.pt_exchange()
+    assert np.array_equal(series.cpu().numpy(), np.stack(rows))
+    assert np.array_equal(a.get_state().view(np.uint32), b.get_state().view(np.uint32))
+    assert np.array_equal(a.get_perm(), b.get_perm())
+
+
+# ---- full-size configs, sampled (the launch configuration bench.py times) -----------------------
+@pytest.mark.parametrize("idx,slots", [(3, (0, 17, 31)), (4, (0, 37, 63))])
+def test_full_size_configs_sampled_slots(xy_mod, oracle_mod, idx, slots):
+    """BASELINE.json configs 4 and 5 at full size on the GPU with the default tiling; the oracle
+    re-does Metropolis and over-relaxation for three sampled slots (every site of those slots),
+    and the reduction + exchange for all slots."""
+    cfg = inputs.CONFIGS[idx]
+    L, R = cfg.L, cfg.R
+    xy, ora = make(xy_mod, oracle_mod, L, R, betas=inputs.betas_of(cfg))
+    if cfg.start == "random":
+        xy.init_random()
+        G = xy.get_state()
+        for r in slots:
+            W, i = H.site_words(L, r, 0, H.STREAM_INIT, SEED)
+            w = np.take_along_axis(W, (i & np.uint64(3)).astype(np.int64)[None], axis=0)[0]
+            assert np.array_equal(G[r].view(np.uint32), (H.TWO_PI_F * H.u24(w)).view(np.uint32))
+        del G
+    else:
+        xy.init_ordered(0.0)
+    xy.mcs(3)
+    S, perm = xy.get_state(), xy.get_perm()
+    stats = metropolis_lockstep(xy, ora, S, 3, slots=slots)
+    print(cfg.name, "metropolis", stats)
+    S1 = xy.get_state()
+    stats, S2 = overrelax_lockstep(xy, ora, S1, slots=slots)
+    print(cfg.name, "overrelax", stats)
+    del S, S1
+    ora.set_active_slots(None)
+    ora.set_state(S2); ora.set_perm(perm); ora.set_counters([4, 4, 3]); xy.set_counters([4, 4, 3])
+    print(cfg.name, "measure", P.check_observables(xy.measure(), ora.measure(), L ** 3))
+    tr = ora.enable_trace(pt=True)
+    xy.pt_exchange(); ora.pt_exchange()
+    print(cfg.name, "pt", P.check_pt(xy.get_perm(), ora.get_perm(), tr["pt_p"], tr["pt_u"]))
+
+
+# ---- P7: long-run statistics ---------------------------------------------------------------------
+def _bin_stats(series, n_bins, N):
+    """series [T,R,5] -> per-bin E/N [n_bins,R] and Q2 = <M4>/<M2>^2 [n_bins,R]."""
+    T = series.shape[0] // n_bins * n_bins
+    s = series[-T:].reshape(n_bins, T // n_bins, series.shape[1], 5)
+    e = s[..., 0].mean(axis=1) / N
+    q2 = s[..., 4].mean(axis=1) / s[..., 3].mean(axis=1) ** 2
+    return e, q2
+
+
+@pytest.mark.parametrize("idx,n_mcs,oracle_seed", [(0, 200, SEED), (0, 4000, SEED + 1), (1, 2000, SEED + 1)])
+def test_long_run_statistics(xy_mod, oracle_mod, idx, n_mcs, oracle_seed):
+    """<E>/N and the Binder ratio Q2 per temperature, GPU vs oracle, within 3 sigma.  Both runs
+    start from a random state at MCS 0 and may still drift, so sigma comes from the scatter of
+    the bin-by-bin DIFFERENCES (zero mean whether or not the runs have equilibrated)."""
+    import torch
+    cfg = inputs.CONFIGS[idx]
+    L, R, N = cfg.L, cfg.R, cfg.L ** 3
+    betas = inputs.betas_of(cfg)
+    xy = xy_mod.XY(L, R, betas, SEED)
+    ora = oracle_mod.XYOracle(L, R, betas, oracle_seed, threads=NCPU)
+    xy.init_random(); ora.init_random()
+    series = torch.zeros(n_mcs, R, 5, dtype=torch.float64, device="cuda")
+    xy.mcs(n_mcs, series)
+    g = series.cpu().numpy()
+    o = np.stack([ora.mcs() for _ in range(n_mcs)])
+    keep = n_mcs - n_mcs // 5
+    n_bins = 20
+    ge, gq = _bin_stats(g[-keep:], n_bins, N)
+    oe, oq = _bin_stats(o[-keep:], n_bins, N)
+    worst = 0.0
+    for name, a, b in (("E/N", ge, oe), ("Q2", gq, oq)):
+        d = a - b
+        z = d.mean(axis=0) / (d.std(axis=0, ddof=1) / np.sqrt(n_bins))
+        print(cfg.name, name, "gpu", a.mean(axis=0)[[0, -1]], "oracle", b.mean(axis=0)[[0, -1]], "max|z|", np.abs(z).max())
+        worst = max(worst, float(np.abs(z).max()))
+        # Student-t with 19 dof: 3 sigma two-sided ~ |z| < 3.45; R ranks x 2 observables are tested at once
+        assert np.abs(z).max() < 4.0 and np.sqrt((z ** 2).mean()) < 1.6
+    gm, gpt = xy.get_accept_counts()
+    om, opt = ora.get_accept_counts()
+    assert abs(gm.sum() / om.sum() - 1) < 0.01 and gpt.sum() > 0 and abs(gpt.sum() / max(opt.sum(), 1) - 1) < 0.2
