@@ -59,14 +59,15 @@ enum {
 };
 
 /* Kernel classes reported by xy_get_kernel_times. */
-#define XY_NUM_KERNEL_CLASSES 6
+#define XY_NUM_KERNEL_CLASSES 7
 enum {
     XY_K_METROPOLIS = 0, /* one Metropolis colour pass over all slots (a2)                         */
     XY_K_OVERRELAX = 1,  /* one over-relaxation colour pass over all slots (a3)                    */
     XY_K_MEASURE = 2,    /* the observable reduction over all slots (a4, first stage)              */
     XY_K_FINALIZE = 3,   /* a4 final stage: per-slot sums in fixed order, by-rank output           */
     XY_K_PT = 4,         /* the replica-exchange kernel (a5)                                       */
-    XY_K_OTHER = 5       /* init, fill, layout conversion                                          */
+    XY_K_OTHER = 5,      /* init, fill, layout conversion                                          */
+    XY_K_FIXUP = 6       /* a2: fp64 settlement of the close Metropolis decisions of one colour pass */
 };
 
 /* ---- lifetime ------------------------------------------------------------------------------ */

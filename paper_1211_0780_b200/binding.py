@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libxy_b200.so")
 _lib = None
 
 XY_OPT_TILE_Y, XY_OPT_TILE_Z, XY_OPT_TRACE, XY_OPT_FUSED_MEASURE, XY_OPT_PROFILE = 1, 2, 3, 4, 5
-KERNEL_CLASSES = ("metropolis", "overrelax", "measure", "finalize", "pt", "other")
+KERNEL_CLASSES = ("metropolis", "overrelax", "measure", "finalize", "pt", "other", "fixup")
 NUM_OBS = 5
 
 # name -> (restype, argtypes); tests/test_abi.py checks this table against include/xy.h

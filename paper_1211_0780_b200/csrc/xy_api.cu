@@ -35,7 +35,8 @@ bool shape_ok(int L, int R) { return L >= 8 && L % 8 == 0 && L <= 1024 && R >= 1
 size_t max_tiles(int L) { return (size_t)(L / 8) * (size_t)(L / 2); }
 
 struct WsLayout {
-    size_t obs_rank, obs_slot, partials, betas, beta_of_slot, beta32, slot_at_rank, met_acc, pt_acc, exact, stage, total;
+    size_t obs_rank, obs_slot, partials, betas, beta_of_slot, beta32, slot_at_rank, met_acc, pt_acc, exact, near_ctl, near_queue, stage, total;
+    unsigned int near_cap;
 };
 WsLayout ws_layout(int L, int R) {
     WsLayout w;
@@ -51,6 +52,13 @@ WsLayout ws_layout(int L, int R) {
     w.met_acc = take((size_t)R * 8);
     w.pt_acc = take((size_t)R * 8);
     w.exact = take(8);
+    w.near_ctl = take(16);                           // near_count, done_ticket, overflow_flag
+    // capacity of the close-decision queue: 2e-3 of one colour pass (expected load at beta ~ 0.45 is 4e-5)
+    const size_t pass_sites = (size_t)R * L * L * L / 2;
+    size_t cap = (size_t)((double)pass_sites * 2e-3);
+    if (cap < 4096) cap = 4096;
+    w.near_cap = (unsigned int)cap;
+    w.near_queue = take(cap * 16);
     w.stage = take((size_t)L * L * L * 4);
     w.total = o;
     return w;
@@ -134,11 +142,17 @@ bool tiles_ok(int L, int TY, int TZ) {
            (size_t)32 * (TY + 2) * (L / 2) <= 200 * 1024;
 }
 
-template <int MODE, bool TRACE>
-int launch_sweep(xy_ctx* c, const SweepParams& P) {
+// The warp-uniform parity mapping needs whole warps per parity class of rows and an even march.
+bool uniform_ok(const SweepParams& P) {
+    const int n = P.nItems;
+    return (P.TY % 2 == 0) && (P.TZ % 2 == 0) && ((n / 2) % 32 == 0) && n >= 64;
+}
+
+template <int MODE, bool TRACE, bool FUSED, bool UNI, bool EXACT_INLINE>
+int launch_sweep_impl(xy_ctx* c, const SweepParams& P) {
     static bool attr_set = false;
     if (!attr_set) {
-        CK(cudaFuncSetAttribute(sweep_kernel<MODE, TRACE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        CK(cudaFuncSetAttribute(sweep_kernel<MODE, TRACE, FUSED, UNI, EXACT_INLINE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_set = true;
     }
     const size_t smem = (size_t)32 * (P.TY + 2) * P.W;
@@ -147,10 +161,26 @@ int launch_sweep(xy_ctx* c, const SweepParams& P) {
     dim3 grid(P.nTY * P.nTZ, c->R);
     {
         LaunchSpan span(c, MODE == MODE_MET ? XY_K_METROPOLIS : MODE == MODE_OR ? XY_K_OVERRELAX : XY_K_MEASURE);
-        sweep_kernel<MODE, TRACE><<<grid, threads, smem, c->stream>>>(P);
+        sweep_kernel<MODE, TRACE, FUSED, UNI, EXACT_INLINE><<<grid, threads, smem, c->stream>>>(P);
     }
     CK(cudaGetLastError());
     return XY_OK;
+}
+
+template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE = false>
+int launch_sweep(xy_ctx* c, const SweepParams& P) {
+    return uniform_ok(P) ? launch_sweep_impl<MODE, TRACE, FUSED, true, EXACT_INLINE>(c, P)
+                         : launch_sweep_impl<MODE, TRACE, FUSED, false, EXACT_INLINE>(c, P);
+}
+
+// True when so many Metropolis decisions would fall inside the fp64 window (|beta| large) that the
+// close-decision queue could overflow: the sweep then re-evaluates them in the loop instead.
+bool need_inline_exact(const xy_ctx* c) {
+    double bmax = 0.0;
+    for (double b : c->betas) bmax = std::fmax(bmax, std::fabs((double)(float)b));
+    const double window = bmax * (double)kWindowPerBeta + (double)kWindowAbs;
+    const double pass_sites = (double)c->R * (double)c->N / 2.0;
+    return (2.0 * window + 6e-8) * pass_sites > (double)c->ws.near_cap / 8.0;
 }
 
 SweepParams base_params(xy_ctx* c, int colour) {
@@ -162,12 +192,15 @@ SweepParams base_params(xy_ctx* c, int colour) {
     P.TY = c->TY; P.TZ = c->TZ; P.nTY = c->L / c->TY; P.nTZ = c->L / c->TZ;
     P.colour = colour;
     P.nItems = P.TY * P.W4;
-    P.half_n = c->half_n;
+    P.half_n = (unsigned int)c->half_n;
     P.keys = c->keys;
     P.beta32_of_slot = c->ws_ptr<float>(c->ws.beta32);
     P.met_acc = c->ws_ptr<unsigned long long>(c->ws.met_acc);
     P.exact_count = c->ws_ptr<unsigned long long>(c->ws.exact);
     P.partials = c->ws_ptr<double>(c->ws.partials);
+    P.near_queue = c->ws_ptr<uint4>(c->ws.near_queue);
+    P.near_count = c->ws_ptr<unsigned int>(c->ws.near_ctl);
+    P.near_cap = c->ws.near_cap;
     return P;
 }
 
@@ -192,6 +225,16 @@ int upload_labels(xy_ctx* c, const int* perm) {
     return XY_OK;
 }
 
+// After a stream synchronise: fail loudly if a colour pass ever produced more close decisions than
+// the queue holds (then some decisions kept their fp32 value; see need_inline_exact).
+int check_near_overflow(xy_ctx* c) {
+    unsigned int flag = 0;
+    CK(cudaMemcpyAsync(&flag, c->ws_ptr<unsigned int>(c->ws.near_ctl) + 2, 4, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    if (flag) return fail(XY_ERR_CUDA, "Metropolis close-decision queue overflowed (capacity %u): results are not exact", c->ws.near_cap);
+    return XY_OK;
+}
+
 int grid_for(size_t n_items, int threads) {
     size_t b = (n_items + threads - 1) / threads;
     const size_t cap = 148 * 16;
@@ -201,7 +244,7 @@ int grid_for(size_t n_items, int threads) {
 int run_measure(xy_ctx* c, double* d_series_row) {
     if (!c->partials_valid) {
         SweepParams P = base_params(c, 1);     // own = white, staged = black
-        int rc = launch_sweep<MODE_MEASURE, false>(c, P);
+        int rc = launch_sweep<MODE_MEASURE, false, false>(c, P);
         if (rc) return rc;
         c->partials_valid = true;
         c->rank_valid = false;
@@ -352,8 +395,24 @@ int xy_metropolis_sweep(xy_ctx* c) {
         SweepParams P = base_params(c, colour);
         P.sweep = c->n_met;
         P.trace = c->d_trace;
-        int rc = c->trace ? launch_sweep<MODE_MET, true>(c, P) : launch_sweep<MODE_MET, false>(c, P);
+        const bool inl = need_inline_exact(c);
+        int rc = inl ? (c->trace ? launch_sweep<MODE_MET, true, false, true>(c, P) : launch_sweep<MODE_MET, false, false, true>(c, P))
+                     : (c->trace ? launch_sweep<MODE_MET, true, false, false>(c, P) : launch_sweep<MODE_MET, false, false, false>(c, P));
         if (rc) return rc;
+        if (!inl) {                                  // settle the close decisions before the next pass reads this colour
+            FixupParams F;
+            memset(&F, 0, sizeof(F));
+            F.own = P.own; F.other = P.other; F.L = c->L; F.W = c->L / 2; F.colour = colour; F.R = c->R;
+            F.half_n = P.half_n; F.keys = c->keys; F.sweep = c->n_met; F.beta32_of_slot = P.beta32_of_slot;
+            F.met_acc = P.met_acc; F.exact_count = P.exact_count; F.near_queue = P.near_queue;
+            F.near_count = P.near_count; F.near_cap = P.near_cap;
+            F.done_ticket = P.near_count + 1; F.overflow_flag = P.near_count + 2;
+            {
+                LaunchSpan span(c, XY_K_FIXUP);
+                met_fixup_kernel<<<148, 256, 0, c->stream>>>(F);
+            }
+            CK(cudaGetLastError());
+        }
     }
     ++c->n_met;
     c->partials_valid = false;
@@ -364,11 +423,13 @@ int xy_overrelax_sweep(xy_ctx* c) {
     if (int rc = need(c)) return rc;
     for (int colour = 0; colour < 2; ++colour) {
         SweepParams P = base_params(c, colour);
-        int rc = launch_sweep<MODE_OR, false>(c, P);
+        const bool fuse = c->fused && colour == 1;      // the white pass sees the final black sites
+        int rc = fuse ? launch_sweep<MODE_OR, false, true>(c, P) : launch_sweep<MODE_OR, false, false>(c, P);
         if (rc) return rc;
     }
     ++c->n_or;
-    c->partials_valid = false;
+    c->partials_valid = c->fused != 0;
+    c->rank_valid = false;
     return XY_OK;
 }
 
@@ -377,7 +438,7 @@ int xy_measure(xy_ctx* c, double* out) {
     if (int rc = run_measure(c, nullptr)) return rc;
     if (out) {
         CK(cudaMemcpyAsync(out, c->ws_ptr<double>(c->ws.obs_rank), (size_t)c->R * 5 * 8, cudaMemcpyDeviceToHost, c->stream));
-        CK(cudaStreamSynchronize(c->stream));
+        return check_near_overflow(c);
     }
     return XY_OK;
 }
@@ -462,8 +523,7 @@ int xy_get_exact_path_count(xy_ctx* c, uint64_t* n) {
     if (int rc = need(c)) return rc;
     if (!n) return fail(XY_ERR_INVALID_ARG, "xy_get_exact_path_count: NULL pointer");
     CK(cudaMemcpyAsync(n, c->ws_ptr<char>(c->ws.exact), 8, cudaMemcpyDeviceToHost, c->stream));
-    CK(cudaStreamSynchronize(c->stream));
-    return XY_OK;
+    return check_near_overflow(c);
 }
 
 int xy_set_option(xy_ctx* c, int option, int value) {
@@ -519,8 +579,7 @@ int xy_get_launch_count(xy_ctx* c, uint64_t* n) {
 
 int xy_synchronize(xy_ctx* c) {
     if (int rc = need(c)) return rc;
-    CK(cudaStreamSynchronize(c->stream));
-    return XY_OK;
+    return check_near_overflow(c);
 }
 
 int xy_debug_get_trace(xy_ctx* c, float* natural) {

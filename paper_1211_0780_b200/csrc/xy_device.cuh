@@ -54,8 +54,8 @@ __device__ __forceinline__ float word_to_u24(uint32_t w) { return (float)(w >> 8
 
 // ---------------------------------------------------------------------------------------------
 // Fast fp32 math.  Stated errors (measured by tests/test_gpu_parity.py::test_device_math_errors
-// against fp64 on [0, 2pi]):  sin/cos abs error <= 1.0e-6 (MUFU.SIN/COS after one FMUL by 1/2pi);
-// atan2 abs error <= 6e-7 rad; ex2.approx relative error <= 2^-22.
+// against fp64 on [0, 2pi]):  sin/cos abs error <= 7.5e-7 (MUFU.SIN/COS after one FMUL by 1/2pi);
+// atan2 abs error <= 8e-7 rad; ex2.approx relative error <= 2^-22.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ void fast_sincos(float x, float& s, float& c) {
     s = __sinf(x);
@@ -127,10 +127,14 @@ __device__ __noinline__ bool metropolis_exact(const float* __restrict__ other, i
     return (double)u < exp(-(double)beta32 * dE);
 }
 
-// Half-width of the window around p_fast inside which the decision is re-evaluated in fp64.
-// The fast path's |p_fast - p_exact| is bounded by beta*(|dh||dS| + |h||d(dS)|) + p*2^-22
-// ~ 0.46*(6e-6*2.9 + 6*2.9e-6) + 2.4e-7 < 1.7e-5 in the very worst case (every one of the 16
-// sin/cos errors at its 1e-6 maximum and aligned); 2^-14 = 6.1e-5 leaves a factor > 3.
-constexpr float kExactWindow = 6.103515625e-05f;
+// Half-width of the window around p_fast inside which the decision is re-evaluated in fp64:
+// window = |beta| * kWindowPerBeta + kWindowAbs.  With e_s = 7.5e-7 the stated sin/cos error, the fast
+// path's g = h.(S' - S) is off by at most |dh||dS| + |h||d(dS)| <= 6 e_s * 2 sqrt2 + 2 e_s * 6 sqrt2
+// = 34 e_s = 2.6e-5 plus fp32 rounding of the six-term sums and the two products (< 8e-6), so
+// |p_fast - p| <= p beta |dg| < beta * 3.4e-5 for p <= 1; ex2.approx and the rounding of its argument
+// add < 1e-6 relative.  kWindowPerBeta = 4e-5 and kWindowAbs = 1.5e-6 leave a margin on both.
+// tests/test_gpu_parity.py::test_fast_path_window measures the actual |p_fast - p_oracle|.
+constexpr float kWindowPerBeta = 4.0e-5f;
+constexpr float kWindowAbs = 1.5e-6f;
 
 }  // namespace xyk
