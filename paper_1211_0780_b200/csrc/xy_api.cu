@@ -32,7 +32,7 @@ int fail(int code, const char* fmt, ...) {
 
 size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 bool shape_ok(int L, int R) { return L >= 8 && L % 8 == 0 && L <= 1024 && R >= 1 && R <= 65535; }
-size_t max_tiles(int L) { return (size_t)(L / 8) * (size_t)(L / 2); }
+size_t max_tiles(int L) { return (size_t)(L / 2) * (size_t)(L / 2); }   // tiles_ok: TY >= 2 and TZ >= 2
 
 struct WsLayout {
     size_t obs_rank, obs_slot, partials, betas, beta_of_slot, beta32, slot_at_rank, met_acc, pt_acc, exact, near_ctl, near_queue, stage, total;
