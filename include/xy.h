@@ -54,8 +54,10 @@ enum {
                               per site (test hook; allocates R*N floats inside the library)         */
     XY_OPT_FUSED_MEASURE = 4, /* 1: the white over-relaxation pass also accumulates the
                               observables, so xy_measure after xy_overrelax_sweep reads no spins    */
-    XY_OPT_PROFILE = 5     /* 1: bracket every kernel launch with a CUDA-event pair on the attached
+    XY_OPT_PROFILE = 5,    /* 1: bracket every kernel launch with a CUDA-event pair on the attached
                               stream; xy_get_kernel_times returns the per-class device times         */
+    XY_OPT_GENERIC_KERNEL = 6 /* 1: always run the colour-pass kernel that reads the row geometry at run
+                              time, also for L = 32, 64, 128, 160 where a compile-time variant exists  */
 };
 
 /* Kernel classes reported by xy_get_kernel_times. */

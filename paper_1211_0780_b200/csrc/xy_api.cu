@@ -81,7 +81,7 @@ struct xy_ctx {
     WsLayout ws;
     float* d_trace = nullptr;
     // options
-    int TY = 0, TZ = 0, trace = 0, fused = 0;
+    int TY = 0, TZ = 0, trace = 0, fused = 0, generic = 0;
     // cache state
     bool partials_valid = false, rank_valid = false;
     uint64_t launches = 0;
@@ -139,38 +139,45 @@ void default_tiles(int L, int R, int& TY, int& TZ) {
 
 bool tiles_ok(int L, int TY, int TZ) {
     return TY >= 2 && TZ >= 2 && L % TY == 0 && L % TZ == 0 && TY * (L / 8) <= 512 &&
-           (size_t)32 * (TY + 2) * (L / 2) <= 200 * 1024;
+           sweep_smem_bytes(L, TY) <= 200 * 1024;
 }
 
-// The warp-uniform parity mapping needs whole warps per parity class of rows and an even march.
-bool uniform_ok(const SweepParams& P) {
-    const int n = P.nItems;
-    return (P.TY % 2 == 0) && (P.TZ % 2 == 0) && ((n / 2) % 32 == 0) && n >= 64;
-}
-
-template <int MODE, bool TRACE, bool FUSED, bool UNI, bool EXACT_INLINE>
+template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE, int W4C>
 int launch_sweep_impl(xy_ctx* c, const SweepParams& P) {
     static bool attr_set = false;
     if (!attr_set) {
-        CK(cudaFuncSetAttribute(sweep_kernel<MODE, TRACE, FUSED, UNI, EXACT_INLINE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        CK(cudaFuncSetAttribute(sweep_kernel<MODE, TRACE, FUSED, EXACT_INLINE, W4C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_set = true;
     }
-    const size_t smem = (size_t)32 * (P.TY + 2) * P.W;
+    const size_t smem = sweep_smem_bytes(P.L, P.TY);
     int threads = P.nItems > 2 * P.W4 ? P.nItems : 2 * P.W4;
     threads = (threads + 31) / 32 * 32;
     dim3 grid(P.nTY * P.nTZ, c->R);
     {
         LaunchSpan span(c, MODE == MODE_MET ? XY_K_METROPOLIS : MODE == MODE_OR ? XY_K_OVERRELAX : XY_K_MEASURE);
-        sweep_kernel<MODE, TRACE, FUSED, UNI, EXACT_INLINE><<<grid, threads, smem, c->stream>>>(P);
+        sweep_kernel<MODE, TRACE, FUSED, EXACT_INLINE, W4C><<<grid, threads, smem, c->stream>>>(P);
     }
     CK(cudaGetLastError());
     return XY_OK;
 }
 
+// Row geometry as a compile-time constant for the lattice sizes of the paper's workloads
+// (L = 32, 64, 128, 160); every other L % 8 == 0 takes the run-time variant of the same kernel.
+// The test hook and the large-|beta| variant are always run-time geometry.
 template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE = false>
 int launch_sweep(xy_ctx* c, const SweepParams& P) {
-    return uniform_ok(P) ? launch_sweep_impl<MODE, TRACE, FUSED, true, EXACT_INLINE>(c, P)
-                         : launch_sweep_impl<MODE, TRACE, FUSED, false, EXACT_INLINE>(c, P);
+    // the compile-time variants want whole warps per row-parity class (warp-uniform x parity)
+    const bool uniform_ok = P.TY % 2 == 0 && (P.nItems / 2) % 32 == 0 && P.nItems >= 64 && P.nItems <= XY_SWEEP_MAX_THREADS;
+    if (!TRACE && !EXACT_INLINE && !c->generic && uniform_ok) {
+        switch (P.W4) {
+            case 4: return launch_sweep_impl<MODE, false, FUSED, false, 4>(c, P);
+            case 8: return launch_sweep_impl<MODE, false, FUSED, false, 8>(c, P);
+            case 16: return launch_sweep_impl<MODE, false, FUSED, false, 16>(c, P);
+            case 20: return launch_sweep_impl<MODE, false, FUSED, false, 20>(c, P);
+            default: break;
+        }
+    }
+    return launch_sweep_impl<MODE, TRACE, FUSED, EXACT_INLINE, 0>(c, P);
 }
 
 // True when so many Metropolis decisions would fall inside the fp64 window (|beta| large) that the
@@ -538,6 +545,7 @@ int xy_set_option(xy_ctx* c, int option, int value) {
         case XY_OPT_TRACE: c->trace = value ? 1 : 0; return XY_OK;
         case XY_OPT_FUSED_MEASURE: c->fused = value ? 1 : 0; return XY_OK;
         case XY_OPT_PROFILE: c->profile = value ? 1 : 0; return XY_OK;
+        case XY_OPT_GENERIC_KERNEL: c->generic = value ? 1 : 0; return XY_OK;
         default: return fail(XY_ERR_INVALID_ARG, "unknown option %d", option);
     }
 }
@@ -550,6 +558,7 @@ int xy_get_option(xy_ctx* c, int option, int* value) {
         case XY_OPT_TRACE: *value = c->trace; return XY_OK;
         case XY_OPT_FUSED_MEASURE: *value = c->fused; return XY_OK;
         case XY_OPT_PROFILE: *value = c->profile; return XY_OK;
+        case XY_OPT_GENERIC_KERNEL: *value = c->generic; return XY_OK;
         default: return fail(XY_ERR_INVALID_ARG, "unknown option %d", option);
     }
 }

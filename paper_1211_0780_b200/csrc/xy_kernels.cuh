@@ -1,315 +1,11 @@
-// xy_kernels.cuh -- the sm_100a kernels of the XY Monte Carlo step.
-//
-// Data layout in HBM: colour-split, replica-major fp32 angles
-//     theta_c[slot][z][y][xh],  c = (x+y+z)&1,  xh = x>>1,  row length W = L/2 floats
-// so a colour pass reads both half-lattices once and writes only its own: 12 B per site-update.
-//
-// One kernel skeleton serves Metropolis (a2), over-relaxation (a3) and the observable reduction
-// (a4).  A thread block owns a tile of TY full rows of its colour and MARCHES through TZ planes.
-// Per plane it (1) turns the other colour's TY+2 rows of the next plane into (cos, sin) ONCE and
-// parks them in a 4-deep ring of shared-memory planes, (2) __syncthreads, (3) updates its own
-// plane from the three staged planes z-1, z, z+1.  Each thread owns four consecutive sites
-// (one 128-bit load and store) of one row for the whole march; x wraps inside the tile, y and z
-// wrap in the global addresses of the staged rows.  The next plane's global loads are issued
-// before the current plane is computed.
+// xy_kernels.cuh -- the small kernels of the XY Monte Carlo step (sm_100a): fp64 settlement of close
+// Metropolis decisions, final reduction stage, replica exchange, start states, layout conversion
+// and the device-math test hooks.  The colour-pass kernel itself is in xy_sweep.cuh.
 #pragma once
 #include "xy_device.cuh"
+#include "xy_sweep.cuh"
 
 namespace xyk {
-
-enum { MODE_MET = 0, MODE_OR = 1, MODE_MEASURE = 2 };
-
-struct SweepParams {
-    float* own;                  // colour array being updated   [R][L][L][W]
-    const float* other;          // the other colour's array (read only during the pass)
-    int L, W, W4;                // W = L/2 floats per row, W4 = L/8 float4 per row
-    int TY, TZ, nTY, nTZ;        // tile rows, march length, tiles per replica in y and z
-    int colour;                  // colour of `own`
-    int nItems;                  // TY * W4 own float4 per plane (<= blockDim.x)
-    unsigned int half_n;         // L^3 / 2 floats per slot per colour
-    PhiloxKeys keys;
-    uint32_t sweep;              // n_met (Philox counter word 2)
-    const float* beta32_of_slot; // Metropolis: fp32 beta label per slot (R13)
-    unsigned long long* met_acc; // Metropolis: accepted proposals per slot
-    unsigned long long* exact_count;  // Metropolis: decisions re-evaluated in fp64
-    float* trace;                // Metropolis test hook: p_fast per own site (same layout as own) or null
-    double* partials;            // measure: [R][nTY*nTZ][3] partial E, Mx, My
-    uint4* near_queue;           // Metropolis: decisions too close to call in fp32 (see met_fixup_kernel)
-    unsigned int* near_count;    // entries appended so far in this colour pass
-    unsigned int near_cap;       // capacity of near_queue
-};
-
-// Two fp32 in one 64-bit register pair: sm_100a has packed fp32 arithmetic (FADD2 / FMUL2 / FFMA2),
-// one issue slot for two additions.  A staged site is the pair (cos theta, sin theta).
-typedef unsigned long long f32x2;
-__device__ __forceinline__ f32x2 pack2(float lo, float hi) { f32x2 d; asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi)); return d; }
-__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
-__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
-
-__device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
-
-// Shared-memory plane: (TY+2) staged rows of the other colour, global rows y0-1 .. y0+TY.  A row of
-// W = 4*W4 sites is stored as two arrays of W4 x 16 bytes: part A holds the (cos, sin) pairs of sites
-// 4q, 4q+1, part B those of sites 4q+2, 4q+3, so that consecutive lanes read consecutive 16-byte
-// words (no bank conflicts) and a thread's four sites are two 128-bit loads.
-//
-// PARMODE: 0 / 1 = the x parity of this thread's own sites is that constant on the first plane of
-// the march and alternates from plane to plane (the launcher maps whole warps to rows of one
-// parity class); 2 = computed per thread and plane (tiles too small for the warp-uniform mapping).
-// EXACT_INLINE (Metropolis only): re-evaluate close decisions in fp64 on the spot (function call in
-// the loop: slow; chosen by the launcher when |beta| is so large that most decisions are "close").
-// Otherwise close decisions are appended to a global queue and settled by met_fixup_kernel, which
-// keeps the fp64 code and its registers out of this loop.
-template <int MODE, bool TRACE, bool FUSED, bool UNI, bool EXACT_INLINE>
-__global__ void __launch_bounds__(512, 2) sweep_kernel(const SweepParams P) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int L = P.L, W = P.W, W4 = P.W4, TY = P.TY, TZ = P.TZ;
-    const int rowB = W * 8;                          // bytes per staged row (W pairs)
-    const int planeB = (TY + 2) * rowB;              // bytes per staged plane; ring of 4 planes
-    const int partB = W4 * 16;                       // byte offset of part B inside a row
-
-    const int tid = threadIdx.x;
-    const int slot = blockIdx.y;
-    const int tile = blockIdx.x;
-    const int tzi = tile / P.nTY, tyi = tile - tzi * P.nTY;
-    const int y0 = tyi * TY, z0 = tzi * TZ;
-
-    const float* __restrict__ other = P.other + (size_t)slot * P.half_n;
-    float* __restrict__ own = P.own + (size_t)slot * P.half_n;
-
-    // ---- this thread's own item: row ty of the tile, float4 column q ---------------------------
-    const bool active = UNI || tid < P.nItems;
-    int ty, q;
-    if (UNI) {                                       // warps [0, n/2) take even rows, the rest odd rows
-        const int half = P.nItems >> 1;
-        const int cls = tid >= half;
-        const int r = tid - (cls ? half : 0);
-        const int t2 = r / W4;
-        ty = 2 * t2 + cls; q = r - t2 * W4;
-    } else {
-        ty = active ? tid / W4 : 0; q = active ? tid - ty * W4 : 0;
-    }
-    const int col = 4 * q;
-    const int y = y0 + ty;
-
-    // staging duty 1: the other colour's float4 at this thread's own (y, q) -> staged row ty+1.
-    // duty 2 (tid < 2*W4): the halo rows, staged row 0 (global y0-1) and TY+1 (global y0+TY).
-    const bool duty2 = tid < 2 * W4;
-    const int r2 = duty2 ? tid / W4 : 0;             // 0 or 1
-    const int q2 = duty2 ? tid - r2 * W4 : 0;
-    int ys2 = r2 ? y0 + TY : y0 - 1;
-    if (ys2 < 0) ys2 += L;
-    if (ys2 >= L) ys2 -= L;
-    const int sOff1 = (ty + 1) * rowB + q * 16;      // byte offset inside a staged plane (part A)
-    const int sOff2 = (r2 ? TY + 1 : 0) * rowB + q2 * 16;
-    const unsigned int planeG = (unsigned int)L * W;
-    const unsigned int gOwn = (unsigned int)y * W + col;       // + z*planeG: this thread's float4 in either colour array
-    const unsigned int gRow2 = (unsigned int)ys2 * W + 4 * q2;
-
-    // measure: which staged items are inside the tile (non-halo) for the other colour's magnetisation
-    constexpr bool MEAS = (MODE == MODE_MEASURE) || FUSED;
-    f32x2 accM = 0ull;                               // per-plane fp32 (Mx, My), flushed to double each plane
-    float accE = 0.f;
-    double dE = 0.0, dMx = 0.0, dMy = 0.0;
-
-    auto plane_of = [&](int j) { int z = z0 - 1 + j; if (z < 0) z += L; if (z >= L) z -= L; return z; };
-    auto stage = [&](const float4& v, int j, int sOff, bool count_m) {
-        float c0, s0, c1, s1, c2, s2, c3, s3;
-        fast_sincos(v.x, s0, c0); fast_sincos(v.y, s1, c1);
-        fast_sincos(v.z, s2, c2); fast_sincos(v.w, s3, c3);
-        const f32x2 p0 = pack2(c0, s0), p1 = pack2(c1, s1), p2 = pack2(c2, s2), p3 = pack2(c3, s3);
-        unsigned char* base = smem_raw + (j & 3) * planeB + sOff;
-        *reinterpret_cast<ulonglong2*>(base) = make_ulonglong2(p0, p1);
-        *reinterpret_cast<ulonglong2*>(base + partB) = make_ulonglong2(p2, p3);
-        if (MEAS && count_m) accM = add2(accM, add2(add2(p0, p1), add2(p2, p3)));
-    };
-
-    // ---- prologue: planes j = 0, 1 staged; j = 2 and own plane 0 in flight -----------------
-    float4 o1 = make_float4(0, 0, 0, 0), o2 = o1, mine = o1;
-#pragma unroll
-    for (int j = 0; j < 2; ++j) {
-        const unsigned int zb = (unsigned int)plane_of(j) * planeG;
-        if (active) { o1 = ldg4(other + zb + gOwn); }
-        if (duty2) { o2 = ldg4(other + zb + gRow2); }
-        if (active) stage(o1, j, sOff1, j >= 1);
-        if (duty2) stage(o2, j, sOff2, false);
-    }
-    {
-        const unsigned int zb = (unsigned int)plane_of(2) * planeG;
-        if (active) { o1 = ldg4(other + zb + gOwn); mine = *reinterpret_cast<const float4*>(own + (unsigned int)z0 * planeG + gOwn); }
-        if (duty2) { o2 = ldg4(other + zb + gRow2); }
-    }
-
-    float bl = 0.f, win24 = 0.f, beta32 = 0.f;
-    if (MODE == MODE_MET) {
-        beta32 = P.beta32_of_slot[slot];
-        bl = beta32 * 1.44269504f;                   // exp(beta g) = 2^(bl g)
-        win24 = (fabsf(beta32) * kWindowPerBeta + kWindowAbs) * 16777216.0f;    // see xy_device.cuh
-    }
-    unsigned int nacc = 0, nexact = 0;
-    const uint32_t quad_row = (uint32_t)(L >> 2);
-    const uint32_t stream = P.colour == 0 ? kStreamMetBlack : kStreamMetWhite;
-    // x parity of this row's own sites on plane z: (y + z + colour) & 1
-    const int par0 = (y + z0 + P.colour) & 1;
-    // edge pair of the row: par = 0 needs site col-1 (part B of column q-1, second pair),
-    // par = 1 needs site col+4 (part A of column q+1, first pair); x wraps inside the row.
-    const int eOff0 = partB + (q == 0 ? W4 - 1 : q - 1) * 16 + 8;
-    const int eOff1 = (q + 1 == W4 ? 0 : q + 1) * 16;
-
-    // ---- one plane of the march ------------------------------------------------------------------
-    auto plane = [&](const int zi, const int par) {
-        const int z = z0 + zi;
-        if (active) stage(o1, zi + 2, sOff1, zi + 2 <= TZ);
-        if (duty2) stage(o2, zi + 2, sOff2, false);
-        const float4 cur = mine;
-        if (zi + 1 < TZ) {                           // prefetch for the next plane
-            const unsigned int zb = (unsigned int)plane_of(zi + 3) * planeG;
-            if (active) { o1 = ldg4(other + zb + gOwn); mine = *reinterpret_cast<const float4*>(own + (unsigned int)(z + 1) * planeG + gOwn); }
-            if (duty2) { o2 = ldg4(other + zb + gRow2); }
-        }
-        __syncthreads();
-        if (active) {
-            const unsigned char* bM = smem_raw + ((zi) & 3) * planeB;       // plane z-1
-            const unsigned char* bZ = smem_raw + ((zi + 1) & 3) * planeB;   // plane z
-            const unsigned char* bP = smem_raw + ((zi + 2) & 3) * planeB;   // plane z+1
-            const int rC = sOff1;                                           // staged row ty+1, part A, column q
-            const ulonglong2 cA = *reinterpret_cast<const ulonglong2*>(bZ + rC);
-            const ulonglong2 cB = *reinterpret_cast<const ulonglong2*>(bZ + rC + partB);
-            const f32x2 e = *reinterpret_cast<const f32x2*>(bZ + (ty + 1) * rowB + (par ? eOff1 : eOff0));
-            const ulonglong2 aA = *reinterpret_cast<const ulonglong2*>(bZ + rC - rowB);
-            const ulonglong2 aB = *reinterpret_cast<const ulonglong2*>(bZ + rC - rowB + partB);
-            const ulonglong2 bA = *reinterpret_cast<const ulonglong2*>(bZ + rC + rowB);
-            const ulonglong2 bB = *reinterpret_cast<const ulonglong2*>(bZ + rC + rowB + partB);
-            const ulonglong2 dA = *reinterpret_cast<const ulonglong2*>(bM + rC);
-            const ulonglong2 dB = *reinterpret_cast<const ulonglong2*>(bM + rC + partB);
-            const ulonglong2 fA = *reinterpret_cast<const ulonglong2*>(bP + rC);
-            const ulonglong2 fB = *reinterpret_cast<const ulonglong2*>(bP + rC + partB);
-            // x neighbours: par = 0 -> sites (j-1, j), par = 1 -> sites (j, j+1) of the same row
-            const f32x2 s01 = add2(cA.x, cA.y), s12 = add2(cA.y, cB.x), s23 = add2(cB.x, cB.y);
-            const f32x2 se = add2(e, par ? cB.y : cA.x);
-            f32x2 h[4];
-            h[0] = add2(add2(par ? s01 : se, add2(aA.x, bA.x)), add2(dA.x, fA.x));
-            h[1] = add2(add2(par ? s12 : s01, add2(aA.y, bA.y)), add2(dA.y, fA.y));
-            h[2] = add2(add2(par ? s23 : s12, add2(aB.x, bB.x)), add2(dB.x, fB.x));
-            h[3] = add2(add2(par ? se : s23, add2(aB.y, bB.y)), add2(dB.y, fB.y));
-            float th[4] = { cur.x, cur.y, cur.z, cur.w };
-            float* const gp = own + (unsigned int)z * planeG + gOwn;
-
-            if (MODE == MODE_MET) {
-                const uint32_t c0 = (uint32_t)(col >> 1) + quad_row * (uint32_t)(y + L * z);
-                float ptrace[4];
-#pragma unroll
-                for (int pr = 0; pr < 2; ++pr) {
-                    uint32_t w[4];
-                    philox4x32_10(c0 + pr, (uint32_t)slot, P.sweep, stream, P.keys, w);
-#pragma unroll
-                    for (int kk = 0; kk < 2; ++kk) {
-                        const int k = 2 * pr + kk;
-                        const float kf = (float)(w[2 * kk] >> 8);
-                        const float tn = kf * kTwoPiU24;
-                        const float uf = (float)(w[2 * kk + 1] >> 8);            // u24 * 2^24
-                        float hx, hy, so, co, sn, cn;
-                        unpack2(h[k], hx, hy);
-                        fast_sincos(th[k], so, co);
-                        fast_sincos(tn, sn, cn);
-                        const float g = fmaf(hx, cn - co, hy * (sn - so));       // = -dE
-                        const float pf = fast_ex2(fmaf(bl, g, 24.0f));            // p * 2^24
-                        bool acc = uf < pf;
-                        if (fabsf(uf - pf) < win24) {
-                            if (EXACT_INLINE) {
-                                acc = metropolis_exact(other, L, W, par, col + k, y, z, th[k], tn, uf * kInvU24, beta32);
-                                ++nexact;
-                            } else {
-                                const unsigned int e = atomicAdd(P.near_count, 1u);
-                                if (e < P.near_cap)
-                                    P.near_queue[e] = make_uint4(((unsigned int)z * planeG + gOwn + k) | (acc ? 0x80000000u : 0u),
-                                                                 (unsigned int)slot, __float_as_uint(th[k]), 0u);
-                            }
-                        }
-                        if (TRACE) ptrace[k] = fminf(pf * kInvU24, 3.0e38f);
-                        if (acc) { th[k] = tn; ++nacc; }
-                    }
-                }
-                if (TRACE) {
-                    float* tr = P.trace + (size_t)P.colour * gridDim.y * P.half_n + (size_t)slot * P.half_n;
-                    *reinterpret_cast<float4*>(tr + (unsigned int)z * planeG + gOwn) = make_float4(ptrace[0], ptrace[1], ptrace[2], ptrace[3]);
-                }
-                *reinterpret_cast<float4*>(gp) = make_float4(th[0], th[1], th[2], th[3]);
-            } else if (MODE == MODE_OR) {
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    float hx, hy;
-                    unpack2(h[k], hx, hy);
-                    if (hx != 0.0f || hy != 0.0f) {                             // R6
-                        float t = fmaf(2.0f, fast_atan2_pos(hy, hx), -th[k]);
-                        t = (t < 0.0f) ? t + kTwoPiF : t;
-                        t = (t >= kTwoPiF) ? t - kTwoPiF : t;
-                        th[k] = t;
-                    }
-                    if (FUSED) {                                                // observables of the NEW state
-                        float s, c;
-                        fast_sincos(th[k], s, c);
-                        accE = fmaf(c, hx, fmaf(s, hy, accE));
-                        accM = add2(accM, pack2(c, s));
-                    }
-                }
-                *reinterpret_cast<float4*>(gp) = make_float4(th[0], th[1], th[2], th[3]);
-            } else {  // MODE_MEASURE: own = white; E = -sum_white S_i . h_i counts every bond once
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    float hx, hy, s, c;
-                    unpack2(h[k], hx, hy);
-                    fast_sincos(th[k], s, c);
-                    accE = fmaf(c, hx, fmaf(s, hy, accE));
-                    accM = add2(accM, pack2(c, s));
-                }
-            }
-        }
-        if (MEAS) {
-            float mx, my;
-            unpack2(accM, mx, my);
-            dE += (double)accE; dMx += (double)mx; dMy += (double)my;
-            accE = 0.f; accM = 0ull;
-        }
-    };
-
-    // ---- march: two planes per iteration so that the parity is a compile-time constant ------------
-    if (UNI) {
-        if (par0) { for (int zi = 0; zi < TZ; zi += 2) { plane(zi, 1); plane(zi + 1, 0); } }
-        else      { for (int zi = 0; zi < TZ; zi += 2) { plane(zi, 0); plane(zi + 1, 1); } }
-    } else {
-        for (int zi = 0; zi < TZ; ++zi) plane(zi, par0 ^ (zi & 1));
-    }
-
-    // ---- epilogue ---------------------------------------------------------------------------
-    if (MODE == MODE_MET) {
-        unsigned int a = nacc, e = nexact;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); e += __shfl_xor_sync(0xffffffffu, e, o); }
-        if ((tid & 31) == 0) {
-            if (a) atomicAdd(P.met_acc + slot, (unsigned long long)a);
-            if (e) atomicAdd(P.exact_count, (unsigned long long)e);
-        }
-    }
-    if (MEAS) {
-        // fixed-order block reduction in double: warp shuffle tree, then warp 0 sums the warps in order
-        __shared__ double red[3][32];
-        double v[3] = { dE, dMx, dMy };
-#pragma unroll
-        for (int c = 0; c < 3; ++c)
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
-        __syncthreads();
-        const int wid = tid >> 5, nw = (blockDim.x + 31) >> 5;
-        if ((tid & 31) == 0) { red[0][wid] = v[0]; red[1][wid] = v[1]; red[2][wid] = v[2]; }
-        __syncthreads();
-        if (tid < 3) {
-            double s = 0.0;
-            for (int k = 0; k < nw; ++k) s += red[tid][k];
-            P.partials[((size_t)slot * gridDim.x + tile) * 3 + tid] = tid == 0 ? -s : s;
-        }
-    }
-}
 
 // Settles the Metropolis decisions the fp32 fast path could not call (|u - p_fast| inside the
 // window of xy_device.cuh): the definition of include/xy.h in fp64 from the STORED angles.  Runs

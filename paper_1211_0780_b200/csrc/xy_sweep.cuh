@@ -1,0 +1,457 @@
+// xy_sweep.cuh -- the colour-pass kernel of the XY Monte Carlo step (sm_100a): Metropolis (a2),
+// over-relaxation (a3, optionally carrying the observables) and the standalone reduction (a4).
+//
+// Data layout in HBM: colour-split, replica-major fp32 angles
+//     theta_c[slot][z][y][xh],  c = (x+y+z)&1,  xh = x>>1,  row length W = L/2 floats
+// so a colour pass reads both half-lattices once and writes only its own: 12 B per site-update.
+//
+// A thread block owns a tile of TY full rows of its colour and MARCHES through TZ planes.  Every
+// thread owns four consecutive sites (one 128-bit load and store) of one row for the whole march.
+// Raw angles travel HBM -> shared memory as bulk asynchronous copies (TMA, cp.async.bulk) issued by
+// one thread kRaw-1 steps ahead into a ring of kRaw raw slots, completing on an mbarrier per slot:
+// per step the other colour's rows y0-1 .. y0+TY of plane z+2 (three copies: the two halo rows
+// wrap in y) and the own colour's TY rows of plane z.  Memory latency is therefore hidden by the
+// copy engine, not by registers or occupancy.  The other colour's raw rows are turned into
+// (cos, sin) pairs ONCE and parked in a 5-deep ring of shared-memory planes while plane z is being
+// updated from the staged planes z-1, z, z+1.  Staging two planes ahead lets the block barrier be
+// split: a thread ARRIVES on an mbarrier right after it has staged and only WAITS for the previous
+// phase at the top of the next step, so warps drift up to one plane apart instead of meeting at a
+// __syncthreads per plane.  x wraps inside the tile, y and z wrap in the source addresses of the
+// copies.  All per-thread addresses are computed once; the march only advances them.
+#pragma once
+#include <type_traits>
+#include "xy_device.cuh"
+
+namespace xyk {
+
+enum { MODE_MET = 0, MODE_OR = 1, MODE_MEASURE = 2 };
+constexpr int kRing = 5;                 // staged (cos, sin) planes resident in shared memory
+constexpr int kRaw = 4;                  // raw-angle slots filled by bulk copies (prefetch distance kRaw-1 steps)
+
+struct SweepParams {
+    float* own;                  // colour array being updated   [R][L][L][W]
+    const float* other;          // the other colour's array (read only during the pass)
+    int L, W, W4;                // W = L/2 floats per row, W4 = L/8 float4 per row
+    int TY, TZ, nTY, nTZ;        // tile rows, march length, tiles per replica in y and z
+    int colour;                  // colour of `own`
+    int nItems;                  // TY * W4 own float4 per plane (<= blockDim.x)
+    unsigned int half_n;         // L^3 / 2 floats per slot per colour
+    PhiloxKeys keys;
+    uint32_t sweep;              // n_met (Philox counter word 2)
+    const float* beta32_of_slot; // Metropolis: fp32 beta label per slot (R13)
+    unsigned long long* met_acc; // Metropolis: accepted proposals per slot
+    unsigned long long* exact_count;  // Metropolis: decisions re-evaluated in fp64
+    float* trace;                // Metropolis test hook: p_fast per own site (same layout as own) or null
+    double* partials;            // measure: [R][nTY*nTZ][3] partial E, Mx, My
+    uint4* near_queue;           // Metropolis: decisions too close to call in fp32 (see met_fixup_kernel)
+    unsigned int* near_count;    // entries appended so far in this colour pass
+    unsigned int near_cap;       // capacity of near_queue
+};
+
+// Two fp32 in one 64-bit register pair: sm_100a has packed fp32 arithmetic (FADD2 / FMUL2 / FFMA2),
+// one issue slot for two additions.  A staged site is the pair (cos theta, sin theta).
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) { f32x2 d; asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi)); return d; }
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+// y + (par ? x1 : x0) as two predicated packed additions (one executes): no 64-bit selects
+__device__ __forceinline__ f32x2 add2_sel(f32x2 y, f32x2 x0, f32x2 x1, int par) {
+    f32x2 d;
+    asm("{\n .reg .pred p;\n setp.ne.s32 p, %4, 0;\n @p add.rn.f32x2 %0, %1, %3;\n @!p add.rn.f32x2 %0, %1, %2;\n}"
+        : "=l"(d) : "l"(y), "l"(x0), "l"(x1), "r"(par));
+    return d;
+}
+
+__device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+
+// ---- mbarrier (shared::cta): the split arrive / wait block barrier -------------------------------
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// try_wait suspends the thread until the phase completes or the hint (ns) expires: no busy spinning
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n .reg .pred p;\n"
+        "XY_WAIT:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
+        " @p bra XY_DONE;\n bra XY_WAIT;\n"
+        "XY_DONE:\n}" ::"r"(bar), "r"(parity), "r"(1000000u) : "memory");
+}
+
+// ---- shared-memory accesses by 32-bit shared-window address (keeps every address a single register
+//      plus an immediate) --------------------------------------------------------------------------
+__device__ __forceinline__ float4 lds_f4(uint32_t a) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ ulonglong2 lds_p2(uint32_t a) {        // two (cos, sin) pairs
+    ulonglong2 v;
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ f32x2 lds_p1(uint32_t a) {
+    f32x2 v;
+    asm volatile("ld.shared.b64 %0, [%1];" : "=l"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts_f4(uint32_t a, float x, float y, float z, float w) {
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a), "f"(x), "f"(y), "f"(z), "f"(w) : "memory");
+}
+// Loop-invariant per-thread values pass through this so that the compiler keeps them in a register
+// instead of recomputing them from the thread index on every step of the march.
+__device__ __forceinline__ void keep(uint32_t& x) { asm volatile("" : "+r"(x)); }
+__device__ __forceinline__ void keep(int& x) { asm volatile("" : "+r"(x)); }
+__device__ __forceinline__ void keep(float& x) { asm volatile("" : "+f"(x)); }
+
+// Appends one close Metropolis decision to the queue settled by met_fixup_kernel (rare path).
+__device__ __noinline__ void push_near(unsigned int* near_count, uint4* near_queue, unsigned int near_cap,
+                                       unsigned int idx_acc, unsigned int slot, float t_old) {
+    const unsigned int e = atomicAdd(near_count, 1u);
+    if (e < near_cap) near_queue[e] = make_uint4(idx_acc, slot, __float_as_uint(t_old), 0u);
+}
+
+// ---- TMA bulk copy global -> shared, completing on an mbarrier ----------------------------------------
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+
+// Shared memory of one block (bytes):  kRing staged planes of (TY+2) rows x W pairs x 8  |
+// kRaw raw slots of (2 TY + 2) rows x W floats x 4 (other colour first, then own)  |  1 + kRaw mbarriers
+__host__ __device__ inline size_t sweep_smem_bytes(int L, int TY) {
+    return (size_t)kRing * (TY + 2) * (L / 2) * 8 + (size_t)kRaw * (2 * TY + 2) * (L / 2) * 4 + 8 * (1 + kRaw) + 8;
+}
+
+// W4C: L/8 as a compile-time constant (row pitches become immediates, and the launcher guarantees
+// whole warps per row-parity class so that the x parity of a warp's sites is uniform) or 0 = read
+// the geometry from P, any tile.
+// EXACT_INLINE (Metropolis only): re-evaluate close decisions in fp64 on the spot (function call in
+// the loop: slow; chosen by the launcher when |beta| is so large that most decisions are "close").
+// Otherwise close decisions are appended to a global queue and settled by met_fixup_kernel, which
+// keeps the fp64 code and its registers out of this loop.
+#ifndef XY_SWEEP_MIN_BLOCKS
+#define XY_SWEEP_MIN_BLOCKS 2
+#endif
+#ifndef XY_SWEEP_MAX_THREADS
+#define XY_SWEEP_MAX_THREADS 320
+#endif
+template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE, int W4C>
+__global__ void __launch_bounds__(W4C ? XY_SWEEP_MAX_THREADS : 512, W4C ? XY_SWEEP_MIN_BLOCKS : 1) sweep_kernel(const SweepParams P) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr bool UNI = W4C != 0;
+    const int L = P.L;
+    const int W4 = W4C ? W4C : P.W4;
+    const int W = 4 * W4;
+    const int TY = P.TY, TZ = P.TZ;
+    const int rowB = W * 8;                          // bytes per staged row (W pairs)
+    const int partB = W4 * 16;                       // byte offset of part B inside a row
+    const int planeB = (TY + 2) * rowB;              // bytes per staged plane; ring of kRing planes
+    const int ringB = kRing * planeB;
+    const int rawRowB = W * 4;                       // bytes per raw row
+    const int rawOwnB = (TY + 2) * rawRowB;          // own rows follow the other colour's TY+2 rows
+    const int rawSlotB = (2 * TY + 2) * rawRowB;
+    const uint32_t sm0 = smem_addr(smem_raw);        // staged ring
+    const uint32_t raw0 = sm0 + ringB;               // raw slots
+    const uint32_t bar = raw0 + kRaw * rawSlotB;     // step barrier, then kRaw "slot full" barriers
+    const uint32_t full0 = bar + 8;
+
+    const int tid = threadIdx.x;
+    const int slot = blockIdx.y;
+    const int tile = blockIdx.x;
+    const int tzi = tile / P.nTY, tyi = tile - tzi * P.nTY;
+    const int y0 = tyi * TY, z0 = tzi * TZ;
+    const int nSteps = TZ + 3;                       // step s stages plane s-1 (relative to z0) and updates plane s-3
+
+    const float* __restrict__ other = P.other + (size_t)slot * P.half_n;
+    float* __restrict__ own = P.own + (size_t)slot * P.half_n;
+    const unsigned int planeG = (unsigned int)L * W;
+
+    // ---- producer: the first lane of the last warp issues all bulk copies of the block -----------
+    const bool producer = tid == (int)blockDim.x - 32;
+    int ylo = y0 - 1, yhi = y0 + TY;
+    if (ylo < 0) ylo += L;
+    if (yhi >= L) yhi -= L;
+    auto issue = [&](int s) {                        // fill raw slot s % kRaw for step s
+        const int rs = s % kRaw;
+        const uint32_t fb = full0 + 8 * rs;
+        const uint32_t dst = raw0 + rs * rawSlotB;
+        const bool has_other = s <= TZ + 1, has_own = s >= 3;
+        mbar_expect_tx(fb, (has_other ? (TY + 2) * rawRowB : 0) + (has_own ? TY * rawRowB : 0));
+        if (has_other) {
+            int z = z0 + s - 1; if (z < 0) z += L; if (z >= L) z -= L;
+            const float* pl = other + (size_t)z * planeG;
+            bulk_g2s(dst, pl + (size_t)ylo * W, rawRowB, fb);
+            bulk_g2s(dst + rawRowB, pl + (size_t)y0 * W, TY * rawRowB, fb);
+            bulk_g2s(dst + (TY + 1) * rawRowB, pl + (size_t)yhi * W, rawRowB, fb);
+        }
+        if (has_own) bulk_g2s(dst + rawOwnB, own + (size_t)(z0 + s - 3) * planeG + (size_t)y0 * W, TY * rawRowB, fb);
+    };
+    if (tid == 0) {
+        mbar_init(bar, blockDim.x);
+        for (int k = 0; k < kRaw; ++k) mbar_init(full0 + 8 * k, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (producer)
+        for (int s = 0; s < kRaw - 1 && s < nSteps; ++s) issue(s);
+
+    // ---- this thread's own item: row ty of the tile, float4 column q; idle threads (block size
+    //      rounded up to a warp) shadow item 0 and store nothing.  UNI: warps [0, n/2) take the
+    //      even rows, the rest the odd rows, so the x parity below is uniform over a warp ----------
+    const bool active = tid < P.nItems;
+    const int item = active ? tid : 0;
+    int ty, q;
+    if (UNI) {
+        const int half = P.nItems >> 1;
+        const int cls = item >= half;
+        const int r = item - (cls ? half : 0);
+        const int t2 = r / W4;
+        ty = 2 * t2 + cls; q = r - t2 * W4;
+    } else {
+        ty = item / W4; q = item - ty * W4;
+    }
+    const int y = y0 + ty;
+
+    // staging duty 1: the other colour's float4 at this thread's own (y, q) -> staged row ty+1.
+    // duty 2 (tid < 2*W4): the halo rows, staged row 0 (global y0-1) and TY+1 (global y0+TY).
+    const bool duty2 = tid < 2 * W4;
+    const int r2 = duty2 ? tid / W4 : 0;             // 0 or 1
+    const int q2 = duty2 ? tid - r2 * W4 : 0;
+    // Staged plane: (TY+2) rows.  A row of W = 4*W4 sites is stored as two arrays of W4 x 16 bytes:
+    // part A holds the (cos, sin) pairs of sites 4q, 4q+1, part B those of sites 4q+2, 4q+3, so
+    // that consecutive lanes read consecutive 16-byte words (no bank conflicts) and a thread's four
+    // sites are two 128-bit loads.
+    uint32_t aRow = sm0 + (ty + 1) * rowB + q * 16;                  // staged row ty+1, part A, column q (+ ring offset)
+    uint32_t aRow2 = sm0 + (r2 ? TY + 1 : 0) * rowB + q2 * 16;
+    uint32_t aRawO = raw0 + ((ty + 1) * W + 4 * q) * 4;              // raw other-colour float4 (+ raw slot offset)
+    uint32_t aRawO2 = raw0 + ((r2 ? TY + 1 : 0) * W + 4 * q2) * 4;
+    uint32_t aRawOwn = raw0 + rawOwnB + (ty * W + 4 * q) * 4;        // raw own-colour float4
+    // edge pair of the row: par = 0 needs site 4q-1 (part B of column q-1, second pair),
+    // par = 1 needs site 4q+4 (part A of column q+1, first pair); x wraps inside the row.
+    uint32_t aEdge0 = sm0 + (ty + 1) * rowB + partB + (q == 0 ? W4 - 1 : q - 1) * 16 + 8;
+    uint32_t aEdge1 = sm0 + (ty + 1) * rowB + (q + 1 == W4 ? 0 : q + 1) * 16;
+    // x parity of this row's own sites on plane z: (y + z + colour) & 1; flips every plane
+    int par = (y + z0 + P.colour) & 1;
+    // Philox counter word 0 of this thread's first quad on plane z0; a plane further is +L*L/4
+    uint32_t ctr0 = (uint32_t)(2 * q) + (uint32_t)(L >> 2) * (uint32_t)(y + L * z0);
+    const uint32_t ctrStep = (uint32_t)(L >> 2) * (uint32_t)L;
+    const unsigned int gOwn = (unsigned int)y * W + 4 * q;
+    unsigned int gz = (unsigned int)z0 * planeG + gOwn;              // element index of the own float4 being updated
+    float* gp = own + gz;                                            // and its address
+    keep(aRow); keep(aRow2); keep(aRawO); keep(aRawO2); keep(aRawOwn); keep(aEdge0); keep(aEdge1); keep(par); keep(ctr0);
+
+    constexpr bool MEAS = (MODE == MODE_MEASURE) || FUSED;
+    f32x2 accM = 0ull;                               // per-plane fp32 (Mx, My), flushed to double each plane
+    float accE = 0.f;
+    double dE = 0.0, dMx = 0.0, dMy = 0.0;
+
+    float bl = 0.f, win24 = 0.f, beta32 = 0.f;
+    PhiloxInv inv = {0u, 0u, 0u, 0u};
+    if (MODE == MODE_MET) {
+        beta32 = P.beta32_of_slot[slot];
+        bl = beta32 * 1.44269504f;                   // exp(beta g) = 2^(bl g)
+        win24 = (fabsf(beta32) * kWindowPerBeta + kWindowAbs) * 16777216.0f;    // see xy_device.cuh
+        inv = philox_block_invariants((uint32_t)slot, P.sweep, P.colour == 0 ? kStreamMetBlack : kStreamMetWhite, P.keys);
+        keep(bl); keep(win24); keep(inv.j0); keep(inv.j1); keep(inv.j2); keep(inv.j3);
+    }
+    unsigned int nacc = 0, nexact = 0;
+    int sS = 0;                                      // ring byte offset of the plane staged this step (slot s % kRing)
+    int rS = 0;                                      // raw byte offset of this step's slot (s % kRaw)
+    uint32_t fullBar = full0;                        // this step's "slot full" barrier and the parity of its phase
+    uint32_t fullPar = 0;
+
+    // raw float4 at `src` -> (cos, sin) of its four angles -> staged plane at `dst`
+    auto stage = [&](uint32_t src, uint32_t dst, bool count_m) {
+        const float4 v = lds_f4(src);
+        float c0, s0, c1, s1, c2, s2, c3, s3;
+        fast_sincos(v.x, s0, c0); fast_sincos(v.y, s1, c1);
+        fast_sincos(v.z, s2, c2); fast_sincos(v.w, s3, c3);
+        sts_f4(dst, c0, s0, c1, s1);
+        sts_f4(dst + partB, c2, s2, c3, s3);
+        if (MEAS && count_m)
+            accM = add2(accM, add2(add2(pack2(c0, s0), pack2(c1, s1)), add2(pack2(c2, s2), pack2(c3, s3))));
+    };
+
+    // One step of the march.  Phase s of the step barrier completes when every thread has arrived s+1
+    // times: once before the march, then once per step after its staging and raw reads.
+    auto step = [&](const int s, auto do_stage, auto do_update) {
+        constexpr bool STAGE = decltype(do_stage)::value, UPDATE = decltype(do_update)::value;
+        // every thread has staged plane s-2, has finished updating plane s-5 (ring slot s % kRing is
+        // free) and has read raw slot (s-1) % kRaw (free for the producer)
+        mbar_wait(bar, (uint32_t)s & 1u);
+        if (producer && s + kRaw - 1 < nSteps) issue(s + kRaw - 1);
+        mbar_wait(fullBar, fullPar);                 // this step's raw rows have landed
+        if (STAGE) {
+            stage(aRawO + rS, aRow + sS, active && s >= 1 && s <= TZ);
+            if (duty2) stage(aRawO2 + rS, aRow2 + sS, false);
+        }
+        float4 cur = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (UPDATE) cur = lds_f4(aRawOwn + rS);
+        mbar_arrive(bar);
+        // ring offsets of planes z+1, z, z-1 (staged one, two and three steps ago)
+        int sP = sS - planeB; if (sP < 0) sP += ringB;
+        int sZ = sP - planeB; if (sZ < 0) sZ += ringB;
+        int sM = sZ - planeB; if (sM < 0) sM += ringB;
+        sS += planeB; if (sS >= ringB) sS = 0;
+        rS += rawSlotB; fullBar += 8;
+        if (rS >= kRaw * rawSlotB) { rS = 0; fullBar = full0; fullPar ^= 1u; }
+        if (!UPDATE) return;
+
+        // ---- local fields of the four own sites from the staged planes z-1, z, z+1 -----------------
+        f32x2 h[4];
+        {
+            const uint32_t aZ = aRow + sZ, aM = aRow + sM, aP = aRow + sP;
+            const ulonglong2 cA = lds_p2(aZ), cB = lds_p2(aZ + partB);
+            const f32x2 e = lds_p1((par ? aEdge1 : aEdge0) + sZ);
+            const ulonglong2 aA = lds_p2(aZ - rowB), aB = lds_p2(aZ - rowB + partB);
+            const ulonglong2 bA = lds_p2(aZ + rowB), bB = lds_p2(aZ + rowB + partB);
+            const ulonglong2 dA = lds_p2(aM), dB = lds_p2(aM + partB);
+            const ulonglong2 fA = lds_p2(aP), fB = lds_p2(aP + partB);
+            const f32x2 y0s = add2(add2(aA.x, bA.x), add2(dA.x, fA.x));
+            const f32x2 y1s = add2(add2(aA.y, bA.y), add2(dA.y, fA.y));
+            const f32x2 y2s = add2(add2(aB.x, bB.x), add2(dB.x, fB.x));
+            const f32x2 y3s = add2(add2(aB.y, bB.y), add2(dB.y, fB.y));
+            // x neighbours: par = 0 -> sites (j-1, j), par = 1 -> sites (j, j+1) of the same row
+            const f32x2 s01 = add2(cA.x, cA.y), s12 = add2(cA.y, cB.x), s23 = add2(cB.x, cB.y);
+            if (UNI) {                               // warp-uniform branch
+                if (par) { h[0] = add2(y0s, s01); h[1] = add2(y1s, s12); h[2] = add2(y2s, s23); h[3] = add2(y3s, add2(cB.y, e)); }
+                else     { h[0] = add2(y0s, add2(e, cA.x)); h[1] = add2(y1s, s01); h[2] = add2(y2s, s12); h[3] = add2(y3s, s23); }
+            } else {
+                const f32x2 se = add2(e, par ? cB.y : cA.x);
+                h[0] = add2(y0s, par ? s01 : se); h[1] = add2(y1s, par ? s12 : s01);
+                h[2] = add2(y2s, par ? s23 : s12); h[3] = add2(y3s, par ? se : s23);
+            }
+        }
+        float th[4] = { cur.x, cur.y, cur.z, cur.w };
+
+        if (MODE == MODE_MET) {
+            float ptrace[4], dist[4];
+#pragma unroll
+            for (int pr = 0; pr < 2; ++pr) {
+                uint32_t w[4];
+                philox4x32_10_var0(ctr0 + pr, inv, P.keys, w);
+#pragma unroll
+                for (int kk = 0; kk < 2; ++kk) {
+                    const int k = 2 * pr + kk;
+                    const float kf = (float)(w[2 * kk] >> 8);
+                    const float tn = kf * kTwoPiU24;
+                    const float uf = (float)(w[2 * kk + 1] >> 8);            // u24 * 2^24
+                    float hx, hy, so, co, sn, cn;
+                    unpack2(h[k], hx, hy);
+                    fast_sincos(th[k], so, co);
+                    fast_sincos(tn, sn, cn);
+                    const float g = fmaf(hx, cn - co, hy * (sn - so));       // = -dE
+                    const float pf = fast_ex2(fmaf(bl, g, 24.0f));            // p * 2^24
+                    bool acc = uf < pf;
+                    dist[k] = fabsf(uf - pf);
+                    if (EXACT_INLINE && dist[k] < win24) {
+                        acc = metropolis_exact(other, L, W, par, 4 * q + k, y, z0 + s - 3, th[k], tn, uf * kInvU24, beta32);
+                        ++nexact;
+                    }
+                    if (TRACE) ptrace[k] = fminf(pf * kInvU24, 3.0e38f);
+                    if (acc) { th[k] = tn; ++nacc; }
+                }
+            }
+            // decisions too close to call in fp32: queue them for met_fixup_kernel (rare)
+            if (!EXACT_INLINE && fminf(fminf(dist[0], dist[1]), fminf(dist[2], dist[3])) < win24 && active) {
+                const float old[4] = { cur.x, cur.y, cur.z, cur.w };
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (dist[k] < win24) {
+                        const bool fast_acc = __float_as_uint(th[k]) != __float_as_uint(old[k]);
+                        push_near(P.near_count, P.near_queue, P.near_cap, (gz + k) | (fast_acc ? 0x80000000u : 0u),
+                                  (unsigned int)slot, old[k]);
+                    }
+            }
+            if (TRACE && active) {
+                float* tr = P.trace + (size_t)P.colour * gridDim.y * P.half_n + (size_t)slot * P.half_n;
+                *reinterpret_cast<float4*>(tr + gz) = make_float4(ptrace[0], ptrace[1], ptrace[2], ptrace[3]);
+            }
+            ctr0 += ctrStep;
+        } else if (MODE == MODE_OR) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                float hx, hy;
+                unpack2(h[k], hx, hy);
+                if (hx != 0.0f || hy != 0.0f) {                             // R6
+                    float t = fmaf(2.0f, fast_atan2_pos(hy, hx), -th[k]);
+                    t = (t < 0.0f) ? t + kTwoPiF : t;
+                    t = (t >= kTwoPiF) ? t - kTwoPiF : t;
+                    th[k] = t;
+                }
+                if (FUSED) {                                                // observables of the NEW state
+                    float sn, cs;
+                    fast_sincos(th[k], sn, cs);
+                    accE = fmaf(cs, hx, fmaf(sn, hy, accE));
+                    accM = add2(accM, pack2(cs, sn));
+                }
+            }
+        } else {  // MODE_MEASURE: own = white; E = -sum_white S_i . h_i counts every bond once
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                float hx, hy, sn, cs;
+                unpack2(h[k], hx, hy);
+                fast_sincos(th[k], sn, cs);
+                accE = fmaf(cs, hx, fmaf(sn, hy, accE));
+                accM = add2(accM, pack2(cs, sn));
+            }
+        }
+        if (MODE != MODE_MEASURE && active) *reinterpret_cast<float4*>(gp) = make_float4(th[0], th[1], th[2], th[3]);
+        if (MEAS) {
+            float mx, my;
+            unpack2(accM, mx, my);
+            if (active) { dE += (double)accE; dMx += (double)mx; dMy += (double)my; }
+            accE = 0.f; accM = 0ull;
+        }
+        gz += planeG;
+        gp += planeG;
+        par ^= 1;
+    };
+
+    // ---- the march: steps 0..2 only stage planes -1, 0, 1; the last step only updates ---------------
+    mbar_arrive(bar);
+    int s = 0;
+#pragma unroll 1
+    for (; s < 3; ++s) step(s, std::true_type{}, std::false_type{});
+#pragma unroll 1
+    for (; s <= TZ + 1; ++s) step(s, std::true_type{}, std::true_type{});
+    step(s, std::false_type{}, std::true_type{});
+
+    // ---- epilogue ---------------------------------------------------------------------------
+    if (MODE == MODE_MET) {
+        unsigned int a = active ? nacc : 0u, e = active ? nexact : 0u;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); e += __shfl_xor_sync(0xffffffffu, e, o); }
+        if ((tid & 31) == 0) {
+            if (a) atomicAdd(P.met_acc + slot, (unsigned long long)a);
+            if (e) atomicAdd(P.exact_count, (unsigned long long)e);
+        }
+    }
+    if (MEAS) {
+        // fixed-order block reduction in double: warp shuffle tree, then warp 0 sums the warps in order
+        __shared__ double red[3][32];
+        double v[3] = { dE, dMx, dMy };
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
+        const int wid = tid >> 5, nw = (blockDim.x + 31) >> 5;
+        if ((tid & 31) == 0) { red[0][wid] = v[0]; red[1][wid] = v[1]; red[2][wid] = v[2]; }
+        __syncthreads();
+        if (tid < 3) {
+            double sum = 0.0;
+            for (int k = 0; k < nw; ++k) sum += red[tid][k];
+            P.partials[((size_t)slot * gridDim.x + tile) * 3 + tid] = tid == 0 ? -sum : sum;
+        }
+    }
+}
+
+}  // namespace xyk
