@@ -438,43 +438,43 @@ def test_full_size_configs_sampled_slots(xy_mod, oracle_mod, idx, slots):
 
 
 # ---- P7: long-run statistics ---------------------------------------------------------------------
-def _bin_stats(series, n_bins, N):
-    """series [T,R,5] -> per-bin E/N [n_bins,R] and Q2 = <M4>/<M2>^2 [n_bins,R]."""
-    T = series.shape[0] // n_bins * n_bins
-    s = series[-T:].reshape(n_bins, T // n_bins, series.shape[1], 5)
-    e = s[..., 0].mean(axis=1) / N
-    q2 = s[..., 4].mean(axis=1) / s[..., 3].mean(axis=1) ** 2
-    return e, q2
+def _run_means(series, N):
+    """series [T,R,5] (after the discarded head) -> time averages E/N [R] and Q2 = <M4>/<M2>^2 [R]."""
+    return series[..., 0].mean(axis=0) / N, series[..., 4].mean(axis=0) / series[..., 3].mean(axis=0) ** 2
 
 
-@pytest.mark.parametrize("idx,n_mcs,oracle_seed", [(0, 200, SEED), (0, 4000, SEED + 1), (1, 2000, SEED + 1)])
-def test_long_run_statistics(xy_mod, oracle_mod, idx, n_mcs, oracle_seed):
-    """<E>/N and the Binder ratio Q2 per temperature, GPU vs oracle, within 3 sigma.  Both runs
-    start from a random state at MCS 0 and may still drift, so sigma comes from the scatter of
-    the bin-by-bin DIFFERENCES (zero mean whether or not the runs have equilibrated)."""
+@pytest.mark.parametrize("idx,n_runs,n_mcs", [(0, 16, 400), (1, 8, 800)])
+def test_long_run_statistics(xy_mod, oracle_mod, idx, n_runs, n_mcs):
+    """<E>/N and the Binder ratio Q2 per temperature, GPU vs oracle, within 3 sigma.  The time series
+    of one run is autocorrelated (and the replicas of one run are coupled by the exchanges), so sigma
+    comes from the scatter over INDEPENDENT runs: n_runs GPU runs and n_runs oracle runs, all with
+    different seeds, each reduced to its time averages after discarding the first quarter; Welch's t
+    per rank, and for the average over ranks."""
     import torch
     cfg = inputs.CONFIGS[idx]
     L, R, N = cfg.L, cfg.R, cfg.L ** 3
     betas = inputs.betas_of(cfg)
-    xy = xy_mod.XY(L, R, betas, SEED)
-    ora = oracle_mod.XYOracle(L, R, betas, oracle_seed, threads=NCPU)
-    xy.init_random(); ora.init_random()
-    series = torch.zeros(n_mcs, R, 5, dtype=torch.float64, device="cuda")
-    xy.mcs(n_mcs, series)
-    g = series.cpu().numpy()
-    o = np.stack([ora.mcs() for _ in range(n_mcs)])
-    keep = n_mcs - n_mcs // 5
-    n_bins = 20
-    ge, gq = _bin_stats(g[-keep:], n_bins, N)
-    oe, oq = _bin_stats(o[-keep:], n_bins, N)
-    worst = 0.0
-    for name, a, b in (("E/N", ge, oe), ("Q2", gq, oq)):
-        d = a - b
-        z = d.mean(axis=0) / (d.std(axis=0, ddof=1) / np.sqrt(n_bins))
-        print(cfg.name, name, "gpu", a.mean(axis=0)[[0, -1]], "oracle", b.mean(axis=0)[[0, -1]], "max|z|", np.abs(z).max())
-        worst = max(worst, float(np.abs(z).max()))
-        # Student-t with 19 dof: 3 sigma two-sided ~ |z| < 3.45; R ranks x 2 observables are tested at once
-        assert np.abs(z).max() < 4.0 and np.sqrt((z ** 2).mean()) < 1.6
+    head = n_mcs // 4
+    G, O = [], []
+    for k in range(n_runs):
+        xy = xy_mod.XY(L, R, betas, SEED + 1000 + k)
+        ora = oracle_mod.XYOracle(L, R, betas, SEED + 2000 + k, threads=NCPU)
+        xy.init_random(); ora.init_random()
+        series = torch.zeros(n_mcs, R, 5, dtype=torch.float64, device="cuda")
+        xy.mcs(n_mcs, series)
+        G.append(_run_means(series.cpu().numpy()[head:], N))
+        O.append(_run_means(np.stack([ora.mcs() for _ in range(n_mcs)])[head:], N))
+    for j, name in enumerate(("E/N", "Q2")):
+        a = np.stack([g[j] for g in G]); b = np.stack([o[j] for o in O])          # [n_runs, R]
+        se = np.sqrt(a.var(axis=0, ddof=1) / n_runs + b.var(axis=0, ddof=1) / n_runs)
+        t = (a.mean(axis=0) - b.mean(axis=0)) / se
+        am, bm = a.mean(axis=1), b.mean(axis=1)                                    # rank averages per run
+        t_all = (am.mean() - bm.mean()) / np.sqrt(am.var(ddof=1) / n_runs + bm.var(ddof=1) / n_runs)
+        print(cfg.name, name, "gpu", a.mean(axis=0)[[0, -1]], "oracle", b.mean(axis=0)[[0, -1]],
+              "se", se[[0, -1]], "max|t|", np.abs(t).max(), "t(rank average)", t_all)
+        # 3 sigma on the rank average (Student-t, >= 14 dof: |t| < 3.5); the R per-rank values are
+        # tested at once, so their bound is wider
+        assert abs(t_all) < 3.5 and np.abs(t).max() < 5.0
     gm, gpt = xy.get_accept_counts()
     om, opt = ora.get_accept_counts()
     assert abs(gm.sum() / om.sum() - 1) < 0.01 and gpt.sum() > 0 and abs(gpt.sum() / max(opt.sum(), 1) - 1) < 0.2
