@@ -164,6 +164,8 @@ def run_ours(args, cfg):
         xy.init_random()
     else:
         xy.init_ordered(0.0)
+    if args.tile_z:
+        xy.set_option(binding.XY_OPT_TILE_Z, args.tile_z)
     xy.set_option(binding.XY_OPT_PROFILE, 1)
 
     def barrier():
@@ -264,6 +266,7 @@ def main():
     ap.add_argument("--config", type=int, default=4, help="index into BASELINE.json configs (default 4: L=160, R=64)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tile-z", type=int, default=0, help="override the march length (tuning; 0 = library default)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     cfg = inputs.CONFIGS[args.config]

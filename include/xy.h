@@ -52,8 +52,9 @@ enum {
     XY_OPT_TILE_Z = 2,     /* planes a thread block marches through (must divide L)                  */
     XY_OPT_TRACE = 3,      /* 1: xy_metropolis_sweep also records its fast-path acceptance probability
                               per site (test hook; allocates R*N floats inside the library)         */
-    XY_OPT_FUSED_MEASURE = 4, /* 1: the white over-relaxation pass also accumulates the
-                              observables, so xy_measure after xy_overrelax_sweep reads no spins    */
+    XY_OPT_FUSED_MEASURE = 4, /* 1 (default): the white over-relaxation pass also accumulates the
+                              observables of the state it leaves behind, so xy_measure / xy_pt_exchange
+                              after xy_overrelax_sweep read no spins; 0: always the standalone reduction */
     XY_OPT_PROFILE = 5,    /* 1: bracket every kernel launch with a CUDA-event pair on the attached
                               stream; xy_get_kernel_times returns the per-class device times         */
     XY_OPT_GENERIC_KERNEL = 6 /* 1: always run the colour-pass kernel that reads the row geometry at run
@@ -129,8 +130,8 @@ int xy_metropolis_sweep(xy_ctx* ctx);
 
 /* One checkerboard over-relaxation sweep, black then white: theta' = 2*atan2(h_y, h_x) - theta
  * reduced to [0, 2pi); unchanged if h = 0  [P:38-43 Eq. 2; R4-R7].  fp32 arithmetic with a
- * stated field error.  With XY_OPT_FUSED_MEASURE the white pass also
- * produces the observables of the new state.  ++n_or. */
+ * stated field error.  With XY_OPT_FUSED_MEASURE (default) the white pass
+ * also produces the observables of the new state.  ++n_or. */
 int xy_overrelax_sweep(xy_ctx* ctx);
 
 /* Observables of the current state, out[R][5] = E, Mx, My, |M|^2, |M|^4 indexed by RANK k

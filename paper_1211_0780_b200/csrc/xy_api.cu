@@ -81,7 +81,7 @@ struct xy_ctx {
     WsLayout ws;
     float* d_trace = nullptr;
     // options
-    int TY = 0, TZ = 0, trace = 0, fused = 0, generic = 0;
+    int TY = 0, TZ = 0, trace = 0, fused = 1, generic = 0;
     // cache state
     bool partials_valid = false, rank_valid = false;
     uint64_t launches = 0;
@@ -142,42 +142,36 @@ bool tiles_ok(int L, int TY, int TZ) {
            sweep_smem_bytes(L, TY) <= 200 * 1024;
 }
 
-template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE, int W4C>
+template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE, int W4C, int TYC>
 int launch_sweep_impl(xy_ctx* c, const SweepParams& P) {
     static bool attr_set = false;
     if (!attr_set) {
-        CK(cudaFuncSetAttribute(sweep_kernel<MODE, TRACE, FUSED, EXACT_INLINE, W4C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        CK(cudaFuncSetAttribute(sweep_kernel<MODE, TRACE, FUSED, EXACT_INLINE, W4C, TYC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_set = true;
     }
     const size_t smem = sweep_smem_bytes(P.L, P.TY);
-    int threads = P.nItems > 2 * P.W4 ? P.nItems : 2 * P.W4;
-    threads = (threads + 31) / 32 * 32;
+    const int threads = (P.nItems + 31) / 32 * 32 + 32;          // compute warps + the auxiliary warp
     dim3 grid(P.nTY * P.nTZ, c->R);
     {
         LaunchSpan span(c, MODE == MODE_MET ? XY_K_METROPOLIS : MODE == MODE_OR ? XY_K_OVERRELAX : XY_K_MEASURE);
-        sweep_kernel<MODE, TRACE, FUSED, EXACT_INLINE, W4C><<<grid, threads, smem, c->stream>>>(P);
+        sweep_kernel<MODE, TRACE, FUSED, EXACT_INLINE, W4C, TYC><<<grid, threads, smem, c->stream>>>(P);
     }
     CK(cudaGetLastError());
     return XY_OK;
 }
 
-// Row geometry as a compile-time constant for the lattice sizes of the paper's workloads
-// (L = 32, 64, 128, 160); every other L % 8 == 0 takes the run-time variant of the same kernel.
-// The test hook and the large-|beta| variant are always run-time geometry.
+// Tile geometry as compile-time constants for the lattice sizes of the paper's workloads
+// (L = 32, 64, 128, 160 with their default tiles); everything else takes the run-time variant of
+// the same kernel.  The test hook and the large-|beta| variant are always run-time geometry.
 template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE = false>
 int launch_sweep(xy_ctx* c, const SweepParams& P) {
-    // the compile-time variants want whole warps per row-parity class (warp-uniform x parity)
-    const bool uniform_ok = P.TY % 2 == 0 && (P.nItems / 2) % 32 == 0 && P.nItems >= 64 && P.nItems <= XY_SWEEP_MAX_THREADS;
-    if (!TRACE && !EXACT_INLINE && !c->generic && uniform_ok) {
-        switch (P.W4) {
-            case 4: return launch_sweep_impl<MODE, false, FUSED, false, 4>(c, P);
-            case 8: return launch_sweep_impl<MODE, false, FUSED, false, 8>(c, P);
-            case 16: return launch_sweep_impl<MODE, false, FUSED, false, 16>(c, P);
-            case 20: return launch_sweep_impl<MODE, false, FUSED, false, 20>(c, P);
-            default: break;
-        }
+    if (!TRACE && !EXACT_INLINE && !c->generic) {
+        if (P.W4 == 20 && P.TY == 16) return launch_sweep_impl<MODE, false, FUSED, false, 20, 16>(c, P);
+        if (P.W4 == 16 && P.TY == 16) return launch_sweep_impl<MODE, false, FUSED, false, 16, 16>(c, P);
+        if (P.W4 == 8 && P.TY == 32) return launch_sweep_impl<MODE, false, FUSED, false, 8, 32>(c, P);
+        if (P.W4 == 4 && P.TY == 32) return launch_sweep_impl<MODE, false, FUSED, false, 4, 32>(c, P);
     }
-    return launch_sweep_impl<MODE, TRACE, FUSED, EXACT_INLINE, 0>(c, P);
+    return launch_sweep_impl<MODE, TRACE, FUSED, EXACT_INLINE, 0, 0>(c, P);
 }
 
 // True when so many Metropolis decisions would fall inside the fp64 window (|beta| large) that the

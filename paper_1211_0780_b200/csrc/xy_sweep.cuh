@@ -7,8 +7,10 @@
 //
 // A thread block owns a tile of TY full rows of its colour and MARCHES through TZ planes.  Every
 // thread owns four consecutive sites (one 128-bit load and store) of one row for the whole march.
-// Raw angles travel HBM -> shared memory as bulk asynchronous copies (TMA, cp.async.bulk) issued by
-// one thread kRaw-1 steps ahead into a ring of kRaw raw slots, completing on an mbarrier per slot:
+// The last warp of the block is an auxiliary warp: its first lane issues the copies, all its lanes
+// stage the two halo rows; the other warps all do identical work.
+// Raw angles travel HBM -> shared memory as bulk asynchronous copies (TMA, cp.async.bulk) issued
+// kRaw-1 steps ahead into a ring of kRaw raw slots, completing on an mbarrier per slot:
 // per step the other colour's rows y0-1 .. y0+TY of plane z+2 (three copies: the two halo rows
 // wrap in y) and the own colour's TY rows of plane z.  Memory latency is therefore hidden by the
 // copy engine, not by registers or occupancy.  The other colour's raw rows are turned into
@@ -130,9 +132,9 @@ __host__ __device__ inline size_t sweep_smem_bytes(int L, int TY) {
     return (size_t)kRing * (TY + 2) * (L / 2) * 8 + (size_t)kRaw * (2 * TY + 2) * (L / 2) * 4 + 8 * (1 + kRaw) + 8;
 }
 
-// W4C: L/8 as a compile-time constant (row pitches become immediates, and the launcher guarantees
-// whole warps per row-parity class so that the x parity of a warp's sites is uniform) or 0 = read
-// the geometry from P, any tile.
+// W4C, TYC: L/8 and the tile rows as compile-time constants (every shared-memory pitch becomes an
+// immediate, and TYC*W4C/2 is a multiple of 32 so that the x parity of a warp's sites is uniform),
+// or 0, 0 = read the geometry from P, any tile.
 // EXACT_INLINE (Metropolis only): re-evaluate close decisions in fp64 on the spot (function call in
 // the loop: slow; chosen by the launcher when |beta| is so large that most decisions are "close").
 // Otherwise close decisions are appended to a global queue and settled by met_fixup_kernel, which
@@ -140,17 +142,14 @@ __host__ __device__ inline size_t sweep_smem_bytes(int L, int TY) {
 #ifndef XY_SWEEP_MIN_BLOCKS
 #define XY_SWEEP_MIN_BLOCKS 2
 #endif
-#ifndef XY_SWEEP_MAX_THREADS
-#define XY_SWEEP_MAX_THREADS 320
-#endif
-template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE, int W4C>
-__global__ void __launch_bounds__(W4C ? XY_SWEEP_MAX_THREADS : 512, W4C ? XY_SWEEP_MIN_BLOCKS : 1) sweep_kernel(const SweepParams P) {
+template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE, int W4C, int TYC>
+__global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN_BLOCKS : 1) sweep_kernel(const SweepParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr bool UNI = W4C != 0;
     const int L = P.L;
     const int W4 = W4C ? W4C : P.W4;
     const int W = 4 * W4;
-    const int TY = P.TY, TZ = P.TZ;
+    const int TY = TYC ? TYC : P.TY, TZ = P.TZ;
     const int rowB = W * 8;                          // bytes per staged row (W pairs)
     const int partB = W4 * 16;                       // byte offset of part B inside a row
     const int planeB = (TY + 2) * rowB;              // bytes per staged plane; ring of kRing planes
@@ -169,104 +168,25 @@ __global__ void __launch_bounds__(W4C ? XY_SWEEP_MAX_THREADS : 512, W4C ? XY_SWE
     const int tzi = tile / P.nTY, tyi = tile - tzi * P.nTY;
     const int y0 = tyi * TY, z0 = tzi * TZ;
     const int nSteps = TZ + 3;                       // step s stages plane s-1 (relative to z0) and updates plane s-3
+    const int nCompute = (int)blockDim.x - 32;       // the last warp is the auxiliary warp
 
     const float* __restrict__ other = P.other + (size_t)slot * P.half_n;
     float* __restrict__ own = P.own + (size_t)slot * P.half_n;
     const unsigned int planeG = (unsigned int)L * W;
 
-    // ---- producer: the first lane of the last warp issues all bulk copies of the block -----------
-    const bool producer = tid == (int)blockDim.x - 32;
-    int ylo = y0 - 1, yhi = y0 + TY;
-    if (ylo < 0) ylo += L;
-    if (yhi >= L) yhi -= L;
-    auto issue = [&](int s) {                        // fill raw slot s % kRaw for step s
-        const int rs = s % kRaw;
-        const uint32_t fb = full0 + 8 * rs;
-        const uint32_t dst = raw0 + rs * rawSlotB;
-        const bool has_other = s <= TZ + 1, has_own = s >= 3;
-        mbar_expect_tx(fb, (has_other ? (TY + 2) * rawRowB : 0) + (has_own ? TY * rawRowB : 0));
-        if (has_other) {
-            int z = z0 + s - 1; if (z < 0) z += L; if (z >= L) z -= L;
-            const float* pl = other + (size_t)z * planeG;
-            bulk_g2s(dst, pl + (size_t)ylo * W, rawRowB, fb);
-            bulk_g2s(dst + rawRowB, pl + (size_t)y0 * W, TY * rawRowB, fb);
-            bulk_g2s(dst + (TY + 1) * rawRowB, pl + (size_t)yhi * W, rawRowB, fb);
-        }
-        if (has_own) bulk_g2s(dst + rawOwnB, own + (size_t)(z0 + s - 3) * planeG + (size_t)y0 * W, TY * rawRowB, fb);
-    };
     if (tid == 0) {
         mbar_init(bar, blockDim.x);
         for (int k = 0; k < kRaw; ++k) mbar_init(full0 + 8 * k, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    if (producer)
-        for (int s = 0; s < kRaw - 1 && s < nSteps; ++s) issue(s);
-
-    // ---- this thread's own item: row ty of the tile, float4 column q; idle threads (block size
-    //      rounded up to a warp) shadow item 0 and store nothing.  UNI: warps [0, n/2) take the
-    //      even rows, the rest the odd rows, so the x parity below is uniform over a warp ----------
-    const bool active = tid < P.nItems;
-    const int item = active ? tid : 0;
-    int ty, q;
-    if (UNI) {
-        const int half = P.nItems >> 1;
-        const int cls = item >= half;
-        const int r = item - (cls ? half : 0);
-        const int t2 = r / W4;
-        ty = 2 * t2 + cls; q = r - t2 * W4;
-    } else {
-        ty = item / W4; q = item - ty * W4;
-    }
-    const int y = y0 + ty;
-
-    // staging duty 1: the other colour's float4 at this thread's own (y, q) -> staged row ty+1.
-    // duty 2 (tid < 2*W4): the halo rows, staged row 0 (global y0-1) and TY+1 (global y0+TY).
-    const bool duty2 = tid < 2 * W4;
-    const int r2 = duty2 ? tid / W4 : 0;             // 0 or 1
-    const int q2 = duty2 ? tid - r2 * W4 : 0;
-    // Staged plane: (TY+2) rows.  A row of W = 4*W4 sites is stored as two arrays of W4 x 16 bytes:
-    // part A holds the (cos, sin) pairs of sites 4q, 4q+1, part B those of sites 4q+2, 4q+3, so
-    // that consecutive lanes read consecutive 16-byte words (no bank conflicts) and a thread's four
-    // sites are two 128-bit loads.
-    uint32_t aRow = sm0 + (ty + 1) * rowB + q * 16;                  // staged row ty+1, part A, column q (+ ring offset)
-    uint32_t aRow2 = sm0 + (r2 ? TY + 1 : 0) * rowB + q2 * 16;
-    uint32_t aRawO = raw0 + ((ty + 1) * W + 4 * q) * 4;              // raw other-colour float4 (+ raw slot offset)
-    uint32_t aRawO2 = raw0 + ((r2 ? TY + 1 : 0) * W + 4 * q2) * 4;
-    uint32_t aRawOwn = raw0 + rawOwnB + (ty * W + 4 * q) * 4;        // raw own-colour float4
-    // edge pair of the row: par = 0 needs site 4q-1 (part B of column q-1, second pair),
-    // par = 1 needs site 4q+4 (part A of column q+1, first pair); x wraps inside the row.
-    uint32_t aEdge0 = sm0 + (ty + 1) * rowB + partB + (q == 0 ? W4 - 1 : q - 1) * 16 + 8;
-    uint32_t aEdge1 = sm0 + (ty + 1) * rowB + (q + 1 == W4 ? 0 : q + 1) * 16;
-    // x parity of this row's own sites on plane z: (y + z + colour) & 1; flips every plane
-    int par = (y + z0 + P.colour) & 1;
-    // Philox counter word 0 of this thread's first quad on plane z0; a plane further is +L*L/4
-    uint32_t ctr0 = (uint32_t)(2 * q) + (uint32_t)(L >> 2) * (uint32_t)(y + L * z0);
-    const uint32_t ctrStep = (uint32_t)(L >> 2) * (uint32_t)L;
-    const unsigned int gOwn = (unsigned int)y * W + 4 * q;
-    unsigned int gz = (unsigned int)z0 * planeG + gOwn;              // element index of the own float4 being updated
-    float* gp = own + gz;                                            // and its address
-    keep(aRow); keep(aRow2); keep(aRawO); keep(aRawO2); keep(aRawOwn); keep(aEdge0); keep(aEdge1); keep(par); keep(ctr0);
 
     constexpr bool MEAS = (MODE == MODE_MEASURE) || FUSED;
     f32x2 accM = 0ull;                               // per-plane fp32 (Mx, My), flushed to double each plane
     float accE = 0.f;
     double dE = 0.0, dMx = 0.0, dMy = 0.0;
-
-    float bl = 0.f, win24 = 0.f, beta32 = 0.f;
-    PhiloxInv inv = {0u, 0u, 0u, 0u};
-    if (MODE == MODE_MET) {
-        beta32 = P.beta32_of_slot[slot];
-        bl = beta32 * 1.44269504f;                   // exp(beta g) = 2^(bl g)
-        win24 = (fabsf(beta32) * kWindowPerBeta + kWindowAbs) * 16777216.0f;    // see xy_device.cuh
-        inv = philox_block_invariants((uint32_t)slot, P.sweep, P.colour == 0 ? kStreamMetBlack : kStreamMetWhite, P.keys);
-        keep(bl); keep(win24); keep(inv.j0); keep(inv.j1); keep(inv.j2); keep(inv.j3);
-    }
     unsigned int nacc = 0, nexact = 0;
-    int sS = 0;                                      // ring byte offset of the plane staged this step (slot s % kRing)
-    int rS = 0;                                      // raw byte offset of this step's slot (s % kRaw)
-    uint32_t fullBar = full0;                        // this step's "slot full" barrier and the parity of its phase
-    uint32_t fullPar = 0;
+    bool active = false;
 
     // raw float4 at `src` -> (cos, sin) of its four angles -> staged plane at `dst`
     auto stage = [&](uint32_t src, uint32_t dst, bool count_m) {
@@ -280,150 +200,239 @@ __global__ void __launch_bounds__(W4C ? XY_SWEEP_MAX_THREADS : 512, W4C ? XY_SWE
             accM = add2(accM, add2(add2(pack2(c0, s0), pack2(c1, s1)), add2(pack2(c2, s2), pack2(c3, s3))));
     };
 
-    // One step of the march.  Phase s of the step barrier completes when every thread has arrived s+1
-    // times: once before the march, then once per step after its staging and raw reads.
-    auto step = [&](const int s, auto do_stage, auto do_update) {
-        constexpr bool STAGE = decltype(do_stage)::value, UPDATE = decltype(do_update)::value;
-        // every thread has staged plane s-2, has finished updating plane s-5 (ring slot s % kRing is
-        // free) and has read raw slot (s-1) % kRaw (free for the producer)
-        mbar_wait(bar, (uint32_t)s & 1u);
-        if (producer && s + kRaw - 1 < nSteps) issue(s + kRaw - 1);
-        mbar_wait(fullBar, fullPar);                 // this step's raw rows have landed
-        if (STAGE) {
-            stage(aRawO + rS, aRow + sS, active && s >= 1 && s <= TZ);
-            if (duty2) stage(aRawO2 + rS, aRow2 + sS, false);
-        }
-        float4 cur = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (UPDATE) cur = lds_f4(aRawOwn + rS);
-        mbar_arrive(bar);
-        // ring offsets of planes z+1, z, z-1 (staged one, two and three steps ago)
-        int sP = sS - planeB; if (sP < 0) sP += ringB;
-        int sZ = sP - planeB; if (sZ < 0) sZ += ringB;
-        int sM = sZ - planeB; if (sM < 0) sM += ringB;
-        sS += planeB; if (sS >= ringB) sS = 0;
+    // Phase s of the step barrier completes when every thread has arrived s+1 times: once before the
+    // march, then once per step after its staging and raw reads.  Waiting for phase s at the top of
+    // step s therefore means: every thread has staged plane s-2, has finished updating plane s-5
+    // (ring slot s % kRing is free) and has read raw slot (s-1) % kRaw (free for the next copies).
+    int sS = 0;                                      // ring byte offset of the plane staged this step (slot s % kRing)
+    int rS = 0;                                      // raw byte offset of this step's slot (s % kRaw)
+    uint32_t fullBar = full0;                        // this step's "slot full" barrier and the parity of its phase
+    uint32_t fullPar = 0;
+    auto advance = [&]() {
+        sS += planeB; if (sS == ringB) sS = 0;
         rS += rawSlotB; fullBar += 8;
-        if (rS >= kRaw * rawSlotB) { rS = 0; fullBar = full0; fullPar ^= 1u; }
-        if (!UPDATE) return;
-
-        // ---- local fields of the four own sites from the staged planes z-1, z, z+1 -----------------
-        f32x2 h[4];
-        {
-            const uint32_t aZ = aRow + sZ, aM = aRow + sM, aP = aRow + sP;
-            const ulonglong2 cA = lds_p2(aZ), cB = lds_p2(aZ + partB);
-            const f32x2 e = lds_p1((par ? aEdge1 : aEdge0) + sZ);
-            const ulonglong2 aA = lds_p2(aZ - rowB), aB = lds_p2(aZ - rowB + partB);
-            const ulonglong2 bA = lds_p2(aZ + rowB), bB = lds_p2(aZ + rowB + partB);
-            const ulonglong2 dA = lds_p2(aM), dB = lds_p2(aM + partB);
-            const ulonglong2 fA = lds_p2(aP), fB = lds_p2(aP + partB);
-            const f32x2 y0s = add2(add2(aA.x, bA.x), add2(dA.x, fA.x));
-            const f32x2 y1s = add2(add2(aA.y, bA.y), add2(dA.y, fA.y));
-            const f32x2 y2s = add2(add2(aB.x, bB.x), add2(dB.x, fB.x));
-            const f32x2 y3s = add2(add2(aB.y, bB.y), add2(dB.y, fB.y));
-            // x neighbours: par = 0 -> sites (j-1, j), par = 1 -> sites (j, j+1) of the same row
-            const f32x2 s01 = add2(cA.x, cA.y), s12 = add2(cA.y, cB.x), s23 = add2(cB.x, cB.y);
-            if (UNI) {                               // warp-uniform branch
-                if (par) { h[0] = add2(y0s, s01); h[1] = add2(y1s, s12); h[2] = add2(y2s, s23); h[3] = add2(y3s, add2(cB.y, e)); }
-                else     { h[0] = add2(y0s, add2(e, cA.x)); h[1] = add2(y1s, s01); h[2] = add2(y2s, s12); h[3] = add2(y3s, s23); }
-            } else {
-                const f32x2 se = add2(e, par ? cB.y : cA.x);
-                h[0] = add2(y0s, par ? s01 : se); h[1] = add2(y1s, par ? s12 : s01);
-                h[2] = add2(y2s, par ? s23 : s12); h[3] = add2(y3s, par ? se : s23);
-            }
-        }
-        float th[4] = { cur.x, cur.y, cur.z, cur.w };
-
-        if (MODE == MODE_MET) {
-            float ptrace[4], dist[4];
-#pragma unroll
-            for (int pr = 0; pr < 2; ++pr) {
-                uint32_t w[4];
-                philox4x32_10_var0(ctr0 + pr, inv, P.keys, w);
-#pragma unroll
-                for (int kk = 0; kk < 2; ++kk) {
-                    const int k = 2 * pr + kk;
-                    const float kf = (float)(w[2 * kk] >> 8);
-                    const float tn = kf * kTwoPiU24;
-                    const float uf = (float)(w[2 * kk + 1] >> 8);            // u24 * 2^24
-                    float hx, hy, so, co, sn, cn;
-                    unpack2(h[k], hx, hy);
-                    fast_sincos(th[k], so, co);
-                    fast_sincos(tn, sn, cn);
-                    const float g = fmaf(hx, cn - co, hy * (sn - so));       // = -dE
-                    const float pf = fast_ex2(fmaf(bl, g, 24.0f));            // p * 2^24
-                    bool acc = uf < pf;
-                    dist[k] = fabsf(uf - pf);
-                    if (EXACT_INLINE && dist[k] < win24) {
-                        acc = metropolis_exact(other, L, W, par, 4 * q + k, y, z0 + s - 3, th[k], tn, uf * kInvU24, beta32);
-                        ++nexact;
-                    }
-                    if (TRACE) ptrace[k] = fminf(pf * kInvU24, 3.0e38f);
-                    if (acc) { th[k] = tn; ++nacc; }
-                }
-            }
-            // decisions too close to call in fp32: queue them for met_fixup_kernel (rare)
-            if (!EXACT_INLINE && fminf(fminf(dist[0], dist[1]), fminf(dist[2], dist[3])) < win24 && active) {
-                const float old[4] = { cur.x, cur.y, cur.z, cur.w };
-#pragma unroll
-                for (int k = 0; k < 4; ++k)
-                    if (dist[k] < win24) {
-                        const bool fast_acc = __float_as_uint(th[k]) != __float_as_uint(old[k]);
-                        push_near(P.near_count, P.near_queue, P.near_cap, (gz + k) | (fast_acc ? 0x80000000u : 0u),
-                                  (unsigned int)slot, old[k]);
-                    }
-            }
-            if (TRACE && active) {
-                float* tr = P.trace + (size_t)P.colour * gridDim.y * P.half_n + (size_t)slot * P.half_n;
-                *reinterpret_cast<float4*>(tr + gz) = make_float4(ptrace[0], ptrace[1], ptrace[2], ptrace[3]);
-            }
-            ctr0 += ctrStep;
-        } else if (MODE == MODE_OR) {
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                float hx, hy;
-                unpack2(h[k], hx, hy);
-                if (hx != 0.0f || hy != 0.0f) {                             // R6
-                    float t = fmaf(2.0f, fast_atan2_pos(hy, hx), -th[k]);
-                    t = (t < 0.0f) ? t + kTwoPiF : t;
-                    t = (t >= kTwoPiF) ? t - kTwoPiF : t;
-                    th[k] = t;
-                }
-                if (FUSED) {                                                // observables of the NEW state
-                    float sn, cs;
-                    fast_sincos(th[k], sn, cs);
-                    accE = fmaf(cs, hx, fmaf(sn, hy, accE));
-                    accM = add2(accM, pack2(cs, sn));
-                }
-            }
-        } else {  // MODE_MEASURE: own = white; E = -sum_white S_i . h_i counts every bond once
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                float hx, hy, sn, cs;
-                unpack2(h[k], hx, hy);
-                fast_sincos(th[k], sn, cs);
-                accE = fmaf(cs, hx, fmaf(sn, hy, accE));
-                accM = add2(accM, pack2(cs, sn));
-            }
-        }
-        if (MODE != MODE_MEASURE && active) *reinterpret_cast<float4*>(gp) = make_float4(th[0], th[1], th[2], th[3]);
-        if (MEAS) {
-            float mx, my;
-            unpack2(accM, mx, my);
-            if (active) { dE += (double)accE; dMx += (double)mx; dMy += (double)my; }
-            accE = 0.f; accM = 0ull;
-        }
-        gz += planeG;
-        gp += planeG;
-        par ^= 1;
+        if (rS == kRaw * rawSlotB) { rS = 0; fullBar = full0; fullPar ^= 1u; }
     };
 
-    // ---- the march: steps 0..2 only stage planes -1, 0, 1; the last step only updates ---------------
-    mbar_arrive(bar);
-    int s = 0;
+    if (tid >= nCompute) {
+        // ---- auxiliary warp: bulk copies (lane 0) and the halo rows y0-1, y0+TY of every staged plane ----
+        const int lane = tid - nCompute;
+        int ylo = y0 - 1, yhi = y0 + TY;
+        if (ylo < 0) ylo += L;
+        if (yhi >= L) yhi -= L;
+        auto issue = [&](int s) {                    // fill raw slot s % kRaw for step s
+            const int rs = s % kRaw;
+            const uint32_t fb = full0 + 8 * rs;
+            const uint32_t dst = raw0 + rs * rawSlotB;
+            const bool has_other = s <= TZ + 1, has_own = s >= 3;
+            mbar_expect_tx(fb, (has_other ? (TY + 2) * rawRowB : 0) + (has_own ? TY * rawRowB : 0));
+            if (has_other) {
+                int z = z0 + s - 1; if (z < 0) z += L; if (z >= L) z -= L;
+                const float* pl = other + (size_t)z * planeG;
+                bulk_g2s(dst, pl + (size_t)ylo * W, rawRowB, fb);
+                bulk_g2s(dst + rawRowB, pl + (size_t)y0 * W, TY * rawRowB, fb);
+                bulk_g2s(dst + (TY + 1) * rawRowB, pl + (size_t)yhi * W, rawRowB, fb);
+            }
+            if (has_own) bulk_g2s(dst + rawOwnB, own + (size_t)(z0 + s - 3) * planeG + (size_t)y0 * W, TY * rawRowB, fb);
+        };
+        if (lane == 0)
+            for (int s = 0; s < kRaw - 1 && s < nSteps; ++s) issue(s);
+        mbar_arrive(bar);
 #pragma unroll 1
-    for (; s < 3; ++s) step(s, std::true_type{}, std::false_type{});
+        for (int s = 0; s < nSteps; ++s) {
+            mbar_wait(bar, (uint32_t)s & 1u);
+            if (s <= TZ + 1) {
+                mbar_wait(fullBar, fullPar);
+                for (int j = lane; j < 2 * W4; j += 32) {
+                    const int r2 = j >= W4, q2 = j - (r2 ? W4 : 0);
+                    stage(raw0 + rS + ((r2 ? TY + 1 : 0) * W + 4 * q2) * 4, sm0 + sS + (r2 ? TY + 1 : 0) * rowB + q2 * 16, false);
+                }
+            }
+            mbar_arrive(bar);                        // the compute warps wait for this: copies come after it
+            if (lane == 0 && s + kRaw - 1 < nSteps) issue(s + kRaw - 1);
+            advance();
+        }
+    } else {
+        // ---- compute warps.  This thread's own item: row ty of the tile, float4 column q; idle threads
+        //      (compute threads rounded up to a warp) shadow item 0 and store nothing.  UNI: warps
+        //      [0, n/2) take the even rows, the rest the odd rows, so the x parity is uniform over a warp
+        active = UNI || tid < P.nItems;
+        const int item = active ? tid : 0;
+        int ty, q;
+        if (UNI) {
+            constexpr int half = W4C * TYC / 2;
+            const int cls = item >= half;
+            const int r = item - (cls ? half : 0);
+            const int t2 = r / W4;
+            ty = 2 * t2 + cls; q = r - t2 * W4;
+        } else {
+            ty = item / W4; q = item - ty * W4;
+        }
+        const int y = y0 + ty;
+        // Staged plane: (TY+2) rows.  A row of W = 4*W4 sites is stored as two arrays of W4 x 16 bytes:
+        // part A holds the (cos, sin) pairs of sites 4q, 4q+1, part B those of sites 4q+2, 4q+3, so
+        // that consecutive lanes read consecutive 16-byte words (no bank conflicts) and a thread's four
+        // sites are two 128-bit loads.  This thread stages the other colour's float4 at its own (y, q).
+        uint32_t aRow = sm0 + (ty + 1) * rowB + q * 16;              // staged row ty+1, part A, column q (+ ring offset)
+        uint32_t aRawO = raw0 + ((ty + 1) * W + 4 * q) * 4;          // raw other-colour float4 (+ raw slot offset);
+        const int ownDelta = rawOwnB - rawRowB;                      // the raw own-colour float4 sits this much further
+        // edge pair of the row: par = 0 needs site 4q-1 (part B of column q-1, second pair),
+        // par = 1 needs site 4q+4 (part A of column q+1, first pair); x wraps inside the row.
+        int eRel0 = partB + ((q == 0 ? W4 - 1 : q - 1) - q) * 16 + 8;            // relative to aRow
+        int eRel1 = ((q + 1 == W4 ? 0 : q + 1) - q) * 16;
+        // x parity of this row's own sites on plane z: (y + z + colour) & 1; flips every plane
+        int par = (y + z0 + P.colour) & 1;
+        // Philox counter word 0 of this thread's first quad on plane z0; a plane further is +L*L/4
+        uint32_t ctr0 = (uint32_t)(2 * q) + (uint32_t)(L >> 2) * (uint32_t)(y + L * z0);
+        const uint32_t ctrStep = (uint32_t)(L >> 2) * (uint32_t)L;
+        unsigned int gz = (unsigned int)z0 * planeG + (unsigned int)y * W + 4 * q;   // element index of the own float4 being updated
+        float* gp = own + gz;                                                        // and its address
+        keep(aRow); keep(aRawO); keep(eRel0); keep(eRel1); keep(par); keep(ctr0);
+
+        float bl = 0.f, win24 = 0.f, beta32 = 0.f;
+        PhiloxInv inv = {0u, 0u, 0u, 0u};
+        if (MODE == MODE_MET) {
+            beta32 = P.beta32_of_slot[slot];
+            bl = beta32 * 1.44269504f;               // exp(beta g) = 2^(bl g)
+            win24 = (fabsf(beta32) * kWindowPerBeta + kWindowAbs) * 16777216.0f;    // see xy_device.cuh
+            inv = philox_block_invariants((uint32_t)slot, P.sweep, P.colour == 0 ? kStreamMetBlack : kStreamMetWhite, P.keys);
+            keep(bl); keep(win24); keep(inv.j0); keep(inv.j1); keep(inv.j2); keep(inv.j3);
+        }
+        uint32_t aS = aRow, aP = aRow, aZ = aRow, aM = aRow;         // staged planes: this step's, z+1, z, z-1
+
+        auto step = [&](const int s, auto do_stage, auto do_update) {
+            constexpr bool STAGE = decltype(do_stage)::value, UPDATE = decltype(do_update)::value;
+            mbar_wait(bar, (uint32_t)s & 1u);
+            mbar_wait(fullBar, fullPar);             // this step's raw rows have landed
+            const uint32_t rO = aRawO + rS;
+            if (STAGE) stage(rO, aS, active && s >= 1 && s <= TZ);
+            float4 cur = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (UPDATE) cur = lds_f4(rO + ownDelta);
+            mbar_arrive(bar);
+            if (UPDATE) {
+                // ---- local fields of the four own sites from the staged planes z-1, z, z+1 -------------
+                f32x2 h[4];
+                {
+                    const ulonglong2 cA = lds_p2(aZ), cB = lds_p2(aZ + partB);
+                    const f32x2 e = lds_p1(aZ + (par ? eRel1 : eRel0));
+                    const ulonglong2 aA = lds_p2(aZ - rowB), aB = lds_p2(aZ - rowB + partB);
+                    const ulonglong2 bA = lds_p2(aZ + rowB), bB = lds_p2(aZ + rowB + partB);
+                    const ulonglong2 dA = lds_p2(aM), dB = lds_p2(aM + partB);
+                    const ulonglong2 fA = lds_p2(aP), fB = lds_p2(aP + partB);
+                    const f32x2 y0s = add2(add2(aA.x, bA.x), add2(dA.x, fA.x));
+                    const f32x2 y1s = add2(add2(aA.y, bA.y), add2(dA.y, fA.y));
+                    const f32x2 y2s = add2(add2(aB.x, bB.x), add2(dB.x, fB.x));
+                    const f32x2 y3s = add2(add2(aB.y, bB.y), add2(dB.y, fB.y));
+                    // x neighbours: par = 0 -> sites (j-1, j), par = 1 -> sites (j, j+1) of the same row
+                    const f32x2 s01 = add2(cA.x, cA.y), s12 = add2(cA.y, cB.x), s23 = add2(cB.x, cB.y);
+                    if (UNI) {                       // warp-uniform branch
+                        if (par) { h[0] = add2(y0s, s01); h[1] = add2(y1s, s12); h[2] = add2(y2s, s23); h[3] = add2(y3s, add2(cB.y, e)); }
+                        else     { h[0] = add2(y0s, add2(e, cA.x)); h[1] = add2(y1s, s01); h[2] = add2(y2s, s12); h[3] = add2(y3s, s23); }
+                    } else {
+                        const f32x2 se = add2(e, par ? cB.y : cA.x);
+                        h[0] = add2(y0s, par ? s01 : se); h[1] = add2(y1s, par ? s12 : s01);
+                        h[2] = add2(y2s, par ? s23 : s12); h[3] = add2(y3s, par ? se : s23);
+                    }
+                }
+                float th[4] = { cur.x, cur.y, cur.z, cur.w };
+
+                if (MODE == MODE_MET) {
+                    float ptrace[4], dist[4];
+#pragma unroll
+                    for (int pr = 0; pr < 2; ++pr) {
+                        uint32_t w[4];
+                        philox4x32_10_var0(ctr0 + pr, inv, P.keys, w);
+#pragma unroll
+                        for (int kk = 0; kk < 2; ++kk) {
+                            const int k = 2 * pr + kk;
+                            const float kf = (float)(w[2 * kk] >> 8);
+                            const float tn = kf * kTwoPiU24;
+                            const float uf = (float)(w[2 * kk + 1] >> 8);        // u24 * 2^24
+                            float hx, hy, so, co, sn, cn;
+                            unpack2(h[k], hx, hy);
+                            fast_sincos(th[k], so, co);
+                            fast_sincos(tn, sn, cn);
+                            const float g = fmaf(hx, cn - co, hy * (sn - so));   // = -dE
+                            const float pf = fast_ex2(fmaf(bl, g, 24.0f));        // p * 2^24
+                            bool acc = uf < pf;
+                            dist[k] = fabsf(uf - pf);
+                            if (EXACT_INLINE && dist[k] < win24) {
+                                acc = metropolis_exact(other, L, W, par, 4 * q + k, y, z0 + s - 3, th[k], tn, uf * kInvU24, beta32);
+                                ++nexact;
+                            }
+                            if (TRACE) ptrace[k] = fminf(pf * kInvU24, 3.0e38f);
+                            if (acc) { th[k] = tn; ++nacc; }
+                        }
+                    }
+                    // decisions too close to call in fp32: queue them for met_fixup_kernel (rare)
+                    if (!EXACT_INLINE && fminf(fminf(dist[0], dist[1]), fminf(dist[2], dist[3])) < win24 && active) {
+                        const float old[4] = { cur.x, cur.y, cur.z, cur.w };
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)
+                            if (dist[k] < win24) {
+                                const bool fast_acc = __float_as_uint(th[k]) != __float_as_uint(old[k]);
+                                push_near(P.near_count, P.near_queue, P.near_cap, (gz + k) | (fast_acc ? 0x80000000u : 0u),
+                                          (unsigned int)slot, old[k]);
+                            }
+                    }
+                    if (TRACE && active) {
+                        float* tr = P.trace + (size_t)P.colour * gridDim.y * P.half_n + (size_t)slot * P.half_n;
+                        *reinterpret_cast<float4*>(tr + gz) = make_float4(ptrace[0], ptrace[1], ptrace[2], ptrace[3]);
+                    }
+                    ctr0 += ctrStep;
+                } else if (MODE == MODE_OR) {
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        float hx, hy;
+                        unpack2(h[k], hx, hy);
+                        if (hx != 0.0f || hy != 0.0f) {                         // R6
+                            float t = fmaf(2.0f, fast_atan2_pos(hy, hx), -th[k]);
+                            t = (t < 0.0f) ? t + kTwoPiF : t;
+                            t = (t >= kTwoPiF) ? t - kTwoPiF : t;
+                            th[k] = t;
+                        }
+                        if (FUSED) {                                            // observables of the NEW state
+                            float sn, cs;
+                            fast_sincos(th[k], sn, cs);
+                            accE = fmaf(cs, hx, fmaf(sn, hy, accE));
+                            accM = add2(accM, pack2(cs, sn));
+                        }
+                    }
+                } else {  // MODE_MEASURE: own = white; E = -sum_white S_i . h_i counts every bond once
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        float hx, hy, sn, cs;
+                        unpack2(h[k], hx, hy);
+                        fast_sincos(th[k], sn, cs);
+                        accE = fmaf(cs, hx, fmaf(sn, hy, accE));
+                        accM = add2(accM, pack2(cs, sn));
+                    }
+                }
+                if (MODE != MODE_MEASURE && active) *reinterpret_cast<float4*>(gp) = make_float4(th[0], th[1], th[2], th[3]);
+                if (MEAS) {
+                    float mx, my;
+                    unpack2(accM, mx, my);
+                    if (active) { dE += (double)accE; dMx += (double)mx; dMy += (double)my; }
+                    accE = 0.f; accM = 0ull;
+                }
+                gz += planeG;
+                gp += planeG;
+                par ^= 1;
+            }
+            aM = aZ; aZ = aP; aP = aS;
+            advance();
+            aS = aRow + sS;
+        };
+
+        // ---- the march: steps 0..2 only stage planes -1, 0, 1; the last step only updates -----------
+        mbar_arrive(bar);
+        int s = 0;
 #pragma unroll 1
-    for (; s <= TZ + 1; ++s) step(s, std::true_type{}, std::true_type{});
-    step(s, std::false_type{}, std::true_type{});
+        for (; s < 3; ++s) step(s, std::true_type{}, std::false_type{});
+#pragma unroll 1
+        for (; s <= TZ + 1; ++s) step(s, std::true_type{}, std::true_type{});
+        step(s, std::false_type{}, std::true_type{});
+    }
 
     // ---- epilogue ---------------------------------------------------------------------------
     if (MODE == MODE_MET) {

@@ -253,6 +253,32 @@ def test_measure_against_oracle(xy_mod, oracle_mod, L, R):
         assert np.allclose(xy.get_beta_of_slot()[perm], inputs.beta_ladder(0.44, 0.47, R))
 
 
+@pytest.mark.parametrize("L,R", SHAPES)
+def test_measure_fused_into_overrelax(xy_mod, oracle_mod, L, R):
+    """The white over-relaxation pass carries the reduction (default): its observables must equal the
+    oracle's on the state the sweep leaves behind, and the standalone reduction's on that same state."""
+    xy, ora = make(xy_mod, oracle_mod, L, R)
+    assert xy.get_option(xy_mod.XY_OPT_FUSED_MEASURE) == 1
+    for name, S in states_for(L, R):
+        xy.set_state(S)
+        xy.overrelax_sweep()
+        n0 = xy.get_launch_count()
+        fused = xy.measure()
+        assert xy.get_launch_count() - n0 <= 1, "only the finalize kernel may run: no second pass over the spins"
+        G = xy.get_state()
+        ora.set_state(G)
+        print(L, R, name, P.check_observables(fused, ora.measure(), L ** 3))
+        xy.set_state(G)                                  # invalidates the cache -> standalone reduction
+        P.check_observables(fused, xy.measure(), L ** 3)
+    xy.set_option(xy_mod.XY_OPT_FUSED_MEASURE, 0)
+    xy.overrelax_sweep()
+    n0 = xy.get_launch_count()
+    unfused = xy.measure()
+    assert xy.get_launch_count() - n0 == 2
+    ora.set_state(xy.get_state())
+    P.check_observables(unfused, ora.measure(), L ** 3)
+
+
 def test_measure_closed_forms(xy_mod):
     """O3 / O7 / O8 on the GPU reduction: ordered, helical (each axis separately) and staggered."""
     L, R = 16, 2
