@@ -74,7 +74,7 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-// try_wait suspends the thread until the phase completes or the hint (ns) expires: no busy spinning
+// try_wait suspends the thread until the phase completes or the time hint (ns) expires
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     asm volatile(
         "{\n .reg .pred p;\n"
@@ -385,12 +385,12 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
                     for (int k = 0; k < 4; ++k) {
                         float hx, hy;
                         unpack2(h[k], hx, hy);
-                        if (hx != 0.0f || hy != 0.0f) {                         // R6
-                            float t = fmaf(2.0f, fast_atan2_pos(hy, hx), -th[k]);
-                            t = (t < 0.0f) ? t + kTwoPiF : t;
-                            t = (t >= kTwoPiF) ? t - kTwoPiF : t;
-                            th[k] = t;
-                        }
+                        // branch-free so that the four sites' dependency chains interleave; h = 0 gives
+                        // NaN through rcp(0) * 0, which the final select discards (R6: spin unchanged)
+                        float t = fmaf(2.0f, fast_atan2_pos(hy, hx), -th[k]);
+                        t = (t < 0.0f) ? t + kTwoPiF : t;
+                        t = (t >= kTwoPiF) ? t - kTwoPiF : t;
+                        th[k] = (fmaxf(fabsf(hx), fabsf(hy)) > 0.0f) ? t : th[k];
                         if (FUSED) {                                            // observables of the NEW state
                             float sn, cs;
                             fast_sincos(th[k], sn, cs);
