@@ -11,15 +11,18 @@
 // stage the two halo rows; the other warps all do identical work.
 // Raw angles travel HBM -> shared memory as bulk asynchronous copies (TMA, cp.async.bulk) issued
 // kRaw-1 steps ahead into a ring of kRaw raw slots, completing on an mbarrier per slot:
-// per step the other colour's rows y0-1 .. y0+TY of plane z+2 (three copies: the two halo rows
+// per step the other colour's rows y0-1 .. y0+TY of plane z+1 (three copies: the two halo rows
 // wrap in y) and the own colour's TY rows of plane z.  Memory latency is therefore hidden by the
-// copy engine, not by registers or occupancy.  The other colour's raw rows are turned into
-// (cos, sin) pairs ONCE and parked in a 5-deep ring of shared-memory planes while plane z is being
-// updated from the staged planes z-1, z, z+1.  Staging two planes ahead lets the block barrier be
-// split: a thread ARRIVES on an mbarrier right after it has staged and only WAITS for the previous
-// phase at the top of the next step, so warps drift up to one plane apart instead of meeting at a
-// __syncthreads per plane.  x wraps inside the tile, y and z wrap in the source addresses of the
-// copies.  All per-thread addresses are computed once; the march only advances them.
+// copy engine, not by registers or occupancy.  Every thread turns the other colour's raw float4 at
+// its own (y, x) position into four (cos, sin) pairs ONCE per plane.  Those pairs are exactly the
+// z neighbours (planes z-1, z+1) and the x neighbours (plane z) of the thread's own four sites, so it
+// keeps them in registers across three steps; shared memory only carries them to the threads of
+// the rows above and below (y neighbours) and to the next column (one edge pair), through a ring of
+// 3 staged planes.  That halves the shared-memory traffic, which is what bounds this kernel next
+// to instruction issue.  The block barrier is split: a thread ARRIVES on an mbarrier right after it
+// has staged plane z+1 and only WAITS for that phase at the top of the next step, so warps drift up
+// to one plane apart instead of meeting at a __syncthreads per plane.  x wraps inside the tile, y
+// and z wrap in the source addresses of the copies.  All per-thread addresses are computed once.
 #pragma once
 #include <type_traits>
 #include "xy_device.cuh"
@@ -27,7 +30,7 @@
 namespace xyk {
 
 enum { MODE_MET = 0, MODE_OR = 1, MODE_MEASURE = 2 };
-constexpr int kRing = 5;                 // staged (cos, sin) planes resident in shared memory
+constexpr int kRing = 3;                 // staged (cos, sin) planes resident in shared memory
 constexpr int kRaw = 4;                  // raw-angle slots filled by bulk copies (prefetch distance kRaw-1 steps)
 
 struct SweepParams {
@@ -167,7 +170,7 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
     const int tile = blockIdx.x;
     const int tzi = tile / P.nTY, tyi = tile - tzi * P.nTY;
     const int y0 = tyi * TY, z0 = tzi * TZ;
-    const int nSteps = TZ + 3;                       // step s stages plane s-1 (relative to z0) and updates plane s-3
+    const int nSteps = TZ + 2;                       // step s stages plane s-1 (relative to z0) and updates plane s-2
     const int nCompute = (int)blockDim.x - 32;       // the last warp is the auxiliary warp
 
     const float* __restrict__ other = P.other + (size_t)slot * P.half_n;
@@ -188,22 +191,22 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
     unsigned int nacc = 0, nexact = 0;
     bool active = false;
 
-    // raw float4 at `src` -> (cos, sin) of its four angles -> staged plane at `dst`
-    auto stage = [&](uint32_t src, uint32_t dst, bool count_m) {
+    // raw float4 at `src` -> (cos, sin) of its four angles -> registers pp[] and staged plane at `dst`
+    auto stage = [&](uint32_t src, uint32_t dst, f32x2 (&pp)[4]) {
         const float4 v = lds_f4(src);
         float c0, s0, c1, s1, c2, s2, c3, s3;
         fast_sincos(v.x, s0, c0); fast_sincos(v.y, s1, c1);
         fast_sincos(v.z, s2, c2); fast_sincos(v.w, s3, c3);
         sts_f4(dst, c0, s0, c1, s1);
         sts_f4(dst + partB, c2, s2, c3, s3);
-        if (MEAS && count_m)
-            accM = add2(accM, add2(add2(pack2(c0, s0), pack2(c1, s1)), add2(pack2(c2, s2), pack2(c3, s3))));
+        pp[0] = pack2(c0, s0); pp[1] = pack2(c1, s1); pp[2] = pack2(c2, s2); pp[3] = pack2(c3, s3);
     };
 
     // Phase s of the step barrier completes when every thread has arrived s+1 times: once before the
     // march, then once per step after its staging and raw reads.  Waiting for phase s at the top of
-    // step s therefore means: every thread has staged plane s-2, has finished updating plane s-5
-    // (ring slot s % kRing is free) and has read raw slot (s-1) % kRaw (free for the next copies).
+    // step s therefore means: every thread has staged plane s-2 (the one whose rows this step reads),
+    // has finished updating plane s-4 (ring slot s % kRing is free) and has read raw slot
+    // (s-1) % kRaw (free for the next copies).
     int sS = 0;                                      // ring byte offset of the plane staged this step (slot s % kRing)
     int rS = 0;                                      // raw byte offset of this step's slot (s % kRaw)
     uint32_t fullBar = full0;                        // this step's "slot full" barrier and the parity of its phase
@@ -224,7 +227,7 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
             const int rs = s % kRaw;
             const uint32_t fb = full0 + 8 * rs;
             const uint32_t dst = raw0 + rs * rawSlotB;
-            const bool has_other = s <= TZ + 1, has_own = s >= 3;
+            const bool has_other = true, has_own = s >= 2;
             mbar_expect_tx(fb, (has_other ? (TY + 2) * rawRowB : 0) + (has_own ? TY * rawRowB : 0));
             if (has_other) {
                 int z = z0 + s - 1; if (z < 0) z += L; if (z >= L) z -= L;
@@ -233,7 +236,7 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
                 bulk_g2s(dst + rawRowB, pl + (size_t)y0 * W, TY * rawRowB, fb);
                 bulk_g2s(dst + (TY + 1) * rawRowB, pl + (size_t)yhi * W, rawRowB, fb);
             }
-            if (has_own) bulk_g2s(dst + rawOwnB, own + (size_t)(z0 + s - 3) * planeG + (size_t)y0 * W, TY * rawRowB, fb);
+            if (has_own) bulk_g2s(dst + rawOwnB, own + (size_t)(z0 + s - 2) * planeG + (size_t)y0 * W, TY * rawRowB, fb);
         };
         if (lane == 0)
             for (int s = 0; s < kRaw - 1 && s < nSteps; ++s) issue(s);
@@ -241,12 +244,11 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
 #pragma unroll 1
         for (int s = 0; s < nSteps; ++s) {
             mbar_wait(bar, (uint32_t)s & 1u);
-            if (s <= TZ + 1) {
-                mbar_wait(fullBar, fullPar);
-                for (int j = lane; j < 2 * W4; j += 32) {
-                    const int r2 = j >= W4, q2 = j - (r2 ? W4 : 0);
-                    stage(raw0 + rS + ((r2 ? TY + 1 : 0) * W + 4 * q2) * 4, sm0 + sS + (r2 ? TY + 1 : 0) * rowB + q2 * 16, false);
-                }
+            mbar_wait(fullBar, fullPar);
+            for (int j = lane; j < 2 * W4; j += 32) {
+                const int r2 = j >= W4, q2 = j - (r2 ? W4 : 0);
+                f32x2 pp[4];
+                stage(raw0 + rS + ((r2 ? TY + 1 : 0) * W + 4 * q2) * 4, sm0 + sS + (r2 ? TY + 1 : 0) * rowB + q2 * 16, pp);
             }
             mbar_arrive(bar);                        // the compute warps wait for this: copies come after it
             if (lane == 0 && s + kRaw - 1 < nSteps) issue(s + kRaw - 1);
@@ -298,38 +300,40 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
             inv = philox_block_invariants((uint32_t)slot, P.sweep, P.colour == 0 ? kStreamMetBlack : kStreamMetWhite, P.keys);
             keep(bl); keep(win24); keep(inv.j0); keep(inv.j1); keep(inv.j2); keep(inv.j3);
         }
-        uint32_t aS = aRow, aP = aRow, aZ = aRow, aM = aRow;         // staged planes: this step's, z+1, z, z-1
+        uint32_t aS = aRow, aZ = aRow;                               // staged planes: this step's (z+1) and the previous one (z)
+        // (cos, sin) pairs of the other colour at this thread's own (y, x) position on planes z-1 and z
+        f32x2 pm[4] = {0ull, 0ull, 0ull, 0ull}, pc[4] = {0ull, 0ull, 0ull, 0ull};
 
-        auto step = [&](const int s, auto do_stage, auto do_update) {
-            constexpr bool STAGE = decltype(do_stage)::value, UPDATE = decltype(do_update)::value;
+        auto step = [&](const int s, auto do_update) {
+            constexpr bool UPDATE = decltype(do_update)::value;
             mbar_wait(bar, (uint32_t)s & 1u);
             mbar_wait(fullBar, fullPar);             // this step's raw rows have landed
             const uint32_t rO = aRawO + rS;
-            if (STAGE) stage(rO, aS, active && s >= 1 && s <= TZ);
+            f32x2 pp[4];                             // plane z+1
+            stage(rO, aS, pp);
+            if (MEAS && active && s >= 1 && s <= TZ) accM = add2(accM, add2(add2(pp[0], pp[1]), add2(pp[2], pp[3])));
             float4 cur = make_float4(0.f, 0.f, 0.f, 0.f);
             if (UPDATE) cur = lds_f4(rO + ownDelta);
             mbar_arrive(bar);
             if (UPDATE) {
-                // ---- local fields of the four own sites from the staged planes z-1, z, z+1 -------------
+                // ---- local fields of the four own sites: z neighbours and the row itself from registers,
+                //      y neighbours (rows above and below) and the edge pair from the staged plane z ------
                 f32x2 h[4];
                 {
-                    const ulonglong2 cA = lds_p2(aZ), cB = lds_p2(aZ + partB);
                     const f32x2 e = lds_p1(aZ + (par ? eRel1 : eRel0));
                     const ulonglong2 aA = lds_p2(aZ - rowB), aB = lds_p2(aZ - rowB + partB);
                     const ulonglong2 bA = lds_p2(aZ + rowB), bB = lds_p2(aZ + rowB + partB);
-                    const ulonglong2 dA = lds_p2(aM), dB = lds_p2(aM + partB);
-                    const ulonglong2 fA = lds_p2(aP), fB = lds_p2(aP + partB);
-                    const f32x2 y0s = add2(add2(aA.x, bA.x), add2(dA.x, fA.x));
-                    const f32x2 y1s = add2(add2(aA.y, bA.y), add2(dA.y, fA.y));
-                    const f32x2 y2s = add2(add2(aB.x, bB.x), add2(dB.x, fB.x));
-                    const f32x2 y3s = add2(add2(aB.y, bB.y), add2(dB.y, fB.y));
+                    const f32x2 y0s = add2(add2(aA.x, bA.x), add2(pm[0], pp[0]));
+                    const f32x2 y1s = add2(add2(aA.y, bA.y), add2(pm[1], pp[1]));
+                    const f32x2 y2s = add2(add2(aB.x, bB.x), add2(pm[2], pp[2]));
+                    const f32x2 y3s = add2(add2(aB.y, bB.y), add2(pm[3], pp[3]));
                     // x neighbours: par = 0 -> sites (j-1, j), par = 1 -> sites (j, j+1) of the same row
-                    const f32x2 s01 = add2(cA.x, cA.y), s12 = add2(cA.y, cB.x), s23 = add2(cB.x, cB.y);
+                    const f32x2 s01 = add2(pc[0], pc[1]), s12 = add2(pc[1], pc[2]), s23 = add2(pc[2], pc[3]);
                     if (UNI) {                       // warp-uniform branch
-                        if (par) { h[0] = add2(y0s, s01); h[1] = add2(y1s, s12); h[2] = add2(y2s, s23); h[3] = add2(y3s, add2(cB.y, e)); }
-                        else     { h[0] = add2(y0s, add2(e, cA.x)); h[1] = add2(y1s, s01); h[2] = add2(y2s, s12); h[3] = add2(y3s, s23); }
+                        if (par) { h[0] = add2(y0s, s01); h[1] = add2(y1s, s12); h[2] = add2(y2s, s23); h[3] = add2(y3s, add2(pc[3], e)); }
+                        else     { h[0] = add2(y0s, add2(e, pc[0])); h[1] = add2(y1s, s01); h[2] = add2(y2s, s12); h[3] = add2(y3s, s23); }
                     } else {
-                        const f32x2 se = add2(e, par ? cB.y : cA.x);
+                        const f32x2 se = add2(e, par ? pc[3] : pc[0]);
                         h[0] = add2(y0s, par ? s01 : se); h[1] = add2(y1s, par ? s12 : s01);
                         h[2] = add2(y2s, par ? s23 : s12); h[3] = add2(y3s, par ? se : s23);
                     }
@@ -357,7 +361,7 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
                             bool acc = uf < pf;
                             dist[k] = fabsf(uf - pf);
                             if (EXACT_INLINE && dist[k] < win24) {
-                                acc = metropolis_exact(other, L, W, par, 4 * q + k, y, z0 + s - 3, th[k], tn, uf * kInvU24, beta32);
+                                acc = metropolis_exact(other, L, W, par, 4 * q + k, y, z0 + s - 2, th[k], tn, uf * kInvU24, beta32);
                                 ++nexact;
                             }
                             if (TRACE) ptrace[k] = fminf(pf * kInvU24, 3.0e38f);
@@ -419,19 +423,20 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
                 gp += planeG;
                 par ^= 1;
             }
-            aM = aZ; aZ = aP; aP = aS;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { pm[k] = pc[k]; pc[k] = pp[k]; }
+            aZ = aS;
             advance();
             aS = aRow + sS;
         };
 
-        // ---- the march: steps 0..2 only stage planes -1, 0, 1; the last step only updates -----------
+        // ---- the march: steps 0 and 1 only stage planes -1 and 0 ----------------------------------------
         mbar_arrive(bar);
         int s = 0;
 #pragma unroll 1
-        for (; s < 3; ++s) step(s, std::true_type{}, std::false_type{});
+        for (; s < 2; ++s) step(s, std::false_type{});
 #pragma unroll 1
-        for (; s <= TZ + 1; ++s) step(s, std::true_type{}, std::true_type{});
-        step(s, std::false_type{}, std::true_type{});
+        for (; s < nSteps; ++s) step(s, std::true_type{});
     }
 
     // ---- epilogue ---------------------------------------------------------------------------
