@@ -31,7 +31,8 @@ namespace xyk {
 
 enum { MODE_MET = 0, MODE_OR = 1, MODE_MEASURE = 2 };
 constexpr int kRing = 3;                 // staged (cos, sin) planes resident in shared memory
-constexpr int kRaw = 4;                  // raw-angle slots filled by bulk copies (prefetch distance kRaw-1 steps)
+constexpr int kRaw = 6;                  // raw-angle slots filled by bulk copies (a multiple of kRing: see the march)
+constexpr int kAhead = 3;                // steps between issuing a copy and reading its slot
 
 struct SweepParams {
     float* own;                  // colour array being updated   [R][L][L][W]
@@ -239,7 +240,7 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
             if (has_own) bulk_g2s(dst + rawOwnB, own + (size_t)(z0 + s - 2) * planeG + (size_t)y0 * W, TY * rawRowB, fb);
         };
         if (lane == 0)
-            for (int s = 0; s < kRaw - 1 && s < nSteps; ++s) issue(s);
+            for (int s = 0; s < kAhead && s < nSteps; ++s) issue(s);
         mbar_arrive(bar);
 #pragma unroll 1
         for (int s = 0; s < nSteps; ++s) {
@@ -251,7 +252,7 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
                 stage(raw0 + rS + ((r2 ? TY + 1 : 0) * W + 4 * q2) * 4, sm0 + sS + (r2 ? TY + 1 : 0) * rowB + q2 * 16, pp);
             }
             mbar_arrive(bar);                        // the compute warps wait for this: copies come after it
-            if (lane == 0 && s + kRaw - 1 < nSteps) issue(s + kRaw - 1);
+            if (lane == 0 && s + kAhead < nSteps) issue(s + kAhead);
             advance();
         }
     } else {
@@ -300,16 +301,20 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
             inv = philox_block_invariants((uint32_t)slot, P.sweep, P.colour == 0 ? kStreamMetBlack : kStreamMetWhite, P.keys);
             keep(bl); keep(win24); keep(inv.j0); keep(inv.j1); keep(inv.j2); keep(inv.j3);
         }
-        uint32_t aS = aRow, aZ = aRow;                               // staged planes: this step's (z+1) and the previous one (z)
-        // (cos, sin) pairs of the other colour at this thread's own (y, x) position on planes z-1 and z
-        f32x2 pm[4] = {0ull, 0ull, 0ull, 0ull}, pc[4] = {0ull, 0ull, 0ull, 0ull};
+        // (cos, sin) pairs of the other colour at this thread's own (y, x) position on three consecutive
+        // planes; the roles (z-1, z, z+1) rotate from step to step, so the march is unrolled by three
+        // (J = s % 3 at compile time: staged-ring slot, raw slot J or J+3, and the roles are all static)
+        f32x2 P0[4] = {0ull, 0ull, 0ull, 0ull}, P1[4] = {0ull, 0ull, 0ull, 0ull}, P2[4] = {0ull, 0ull, 0ull, 0ull};
+        int rH = 0;                                  // 0: raw slots 0..2, 1: raw slots 3..5 (toggles every three steps)
 
-        auto step = [&](const int s, auto do_update) {
+        auto step = [&](const int s, auto do_update, auto jc, f32x2 (&pm)[4], f32x2 (&pc)[4], f32x2 (&pp)[4]) {
             constexpr bool UPDATE = decltype(do_update)::value;
+            constexpr int J = decltype(jc)::value;
+            if (J == 0 && s > 0) { rH ^= 1; if (!rH) fullPar ^= 1u; }
+            const uint32_t aS = aRow + J * planeB, aZ = aRow + ((J + 2) % 3) * planeB;   // planes z+1 (staged now) and z
             mbar_wait(bar, (uint32_t)s & 1u);
-            mbar_wait(fullBar, fullPar);             // this step's raw rows have landed
-            const uint32_t rO = aRawO + rS;
-            f32x2 pp[4];                             // plane z+1
+            mbar_wait(full0 + 8 * J + (rH ? 24 : 0), fullPar);       // this step's raw rows have landed
+            const uint32_t rO = aRawO + J * rawSlotB + (rH ? 3 * rawSlotB : 0);
             stage(rO, aS, pp);
             if (MEAS && active && s >= 1 && s <= TZ) accM = add2(accM, add2(add2(pp[0], pp[1]), add2(pp[2], pp[3])));
             float4 cur = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -423,20 +428,23 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
                 gp += planeG;
                 par ^= 1;
             }
-#pragma unroll
-            for (int k = 0; k < 4; ++k) { pm[k] = pc[k]; pc[k] = pp[k]; }
-            aZ = aS;
-            advance();
-            aS = aRow + sS;
         };
 
-        // ---- the march: steps 0 and 1 only stage planes -1 and 0 ----------------------------------------
+        // ---- the march: steps 0 and 1 only stage planes -1 and 0; step s stages into P[s % 3] ------------
         mbar_arrive(bar);
-        int s = 0;
+        using T = std::true_type; using F = std::false_type;
+        using J0 = std::integral_constant<int, 0>; using J1 = std::integral_constant<int, 1>; using J2 = std::integral_constant<int, 2>;
+        step(0, F{}, J0{}, P1, P2, P0);
+        step(1, F{}, J1{}, P2, P0, P1);
+        int s = 2;
 #pragma unroll 1
-        for (; s < 2; ++s) step(s, std::false_type{});
-#pragma unroll 1
-        for (; s < nSteps; ++s) step(s, std::true_type{});
+        for (; s + 3 <= nSteps; s += 3) {
+            step(s, T{}, J2{}, P0, P1, P2);
+            step(s + 1, T{}, J0{}, P1, P2, P0);
+            step(s + 2, T{}, J1{}, P2, P0, P1);
+        }
+        if (s < nSteps) { step(s, T{}, J2{}, P0, P1, P2); ++s; }
+        if (s < nSteps) { step(s, T{}, J0{}, P1, P2, P0); ++s; }
     }
 
     // ---- epilogue ---------------------------------------------------------------------------
