@@ -126,15 +126,17 @@ void default_tiles(int L, int R, int& TY, int& TZ) {
     TY = 8;
     for (int t = 8; t <= L; ++t)
         if (L % t == 0 && t * W4 <= 320) TY = t;
-    // march length: long enough to amortise the two halo planes, short enough for >= ~4 waves of CTAs
+    // March length: a block costs TZ + 2 steps (two of them only stage) and 2 blocks fit an SM, so
+    // the pass takes about ceil(blocks / (2 * 148 SMs)) * (TZ + 1/2) step-times: take the divisor of L
+    // that minimises it (the last, partly filled wave is what a long march wastes).
     TZ = L;
-    const long want = 4L * 148 * 3;
+    double best = 1e300;
     for (int t = L; t >= 8; --t) {
         if (L % t) continue;
-        TZ = t;
-        if ((long)R * (L / TY) * (L / t) >= want) break;
+        const long blocks = (long)R * (L / TY) * (L / t);
+        const double cost = (double)((blocks + 295) / 296) * (t + 0.5);
+        if (cost < best * 0.999) { best = cost; TZ = t; }
     }
-    if (TZ < 8) TZ = L < 8 ? L : 8;
 }
 
 bool tiles_ok(int L, int TY, int TZ) {
@@ -254,7 +256,7 @@ int run_measure(xy_ctx* c, double* d_series_row) {
         const int n_tiles = (c->L / c->TY) * (c->L / c->TZ);
         {
             LaunchSpan span(c, XY_K_FINALIZE);
-            measure_finalize_kernel<<<c->R, 128, 0, c->stream>>>(c->ws_ptr<double>(c->ws.partials), n_tiles,
+            measure_finalize_kernel<<<(c->R + 3) / 4, 128, 0, c->stream>>>(c->ws_ptr<double>(c->ws.partials), n_tiles, c->R,
                                                                  c->ws_ptr<int>(c->ws.slot_at_rank),
                                                                  c->ws_ptr<double>(c->ws.obs_rank),
                                                                  c->ws_ptr<double>(c->ws.obs_slot), d_series_row);
@@ -444,11 +446,26 @@ int xy_measure(xy_ctx* c, double* out) {
     return XY_OK;
 }
 
-int xy_pt_exchange(xy_ctx* c) {
-    if (int rc = need(c)) return rc;
-    if (int rc = run_measure(c, nullptr)) return rc;
-    const int pairs = c->R / 2 + 1;
-    {
+// One exchange; d_series_row (device, R*5 doubles or null) also receives the by-rank observables the
+// decisions were taken on.  When those are not yet reduced to ranks, the final reduction stage and
+// the exchange run as ONE kernel.
+static int pt_exchange_impl(xy_ctx* c, double* d_series_row) {
+    if (!c->partials_valid) {
+        SweepParams P = base_params(c, 1);     // own = white, staged = black
+        if (int rc = launch_sweep<MODE_MEASURE, false, false>(c, P)) return rc;
+        c->partials_valid = true;
+        c->rank_valid = false;
+    }
+    if (!c->rank_valid || d_series_row) {
+        const int n_tiles = (c->L / c->TY) * (c->L / c->TZ);
+        LaunchSpan span(c, XY_K_PT);
+        finalize_pt_kernel<<<1, 1024, 0, c->stream>>>(
+            c->ws_ptr<double>(c->ws.partials), n_tiles, c->R, c->n_pt, c->keys, c->ws_ptr<double>(c->ws.betas),
+            c->ws_ptr<int>(c->ws.slot_at_rank), c->ws_ptr<double>(c->ws.obs_rank), c->ws_ptr<double>(c->ws.obs_slot),
+            d_series_row, c->ws_ptr<double>(c->ws.beta_of_slot), c->ws_ptr<float>(c->ws.beta32),
+            c->ws_ptr<unsigned long long>(c->ws.pt_acc));
+    } else {
+        const int pairs = c->R / 2 + 1;
         LaunchSpan span(c, XY_K_PT);
         pt_exchange_kernel<<<(pairs + 127) / 128, 128, 0, c->stream>>>(
             c->R, c->n_pt, c->keys, c->ws_ptr<double>(c->ws.betas), c->ws_ptr<double>(c->ws.obs_slot),
@@ -457,8 +474,13 @@ int xy_pt_exchange(xy_ctx* c) {
     }
     CK(cudaGetLastError());
     ++c->n_pt;
-    c->rank_valid = false;
+    c->rank_valid = false;                     // the by-rank rows now belong to the previous labelling
     return XY_OK;
+}
+
+int xy_pt_exchange(xy_ctx* c) {
+    if (int rc = need(c)) return rc;
+    return pt_exchange_impl(c, nullptr);
 }
 
 int xy_mcs(xy_ctx* c, int n_mcs, double* d_series) {
@@ -467,8 +489,7 @@ int xy_mcs(xy_ctx* c, int n_mcs, double* d_series) {
     for (int t = 0; t < n_mcs; ++t) {
         if (int rc = xy_metropolis_sweep(c)) return rc;
         if (int rc = xy_overrelax_sweep(c)) return rc;
-        if (int rc = run_measure(c, d_series ? d_series + (size_t)t * c->R * 5 : nullptr)) return rc;
-        if (int rc = xy_pt_exchange(c)) return rc;
+        if (int rc = pt_exchange_impl(c, d_series ? d_series + (size_t)t * c->R * 5 : nullptr)) return rc;
     }
     return XY_OK;
 }

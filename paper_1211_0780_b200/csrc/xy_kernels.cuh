@@ -95,34 +95,35 @@ __global__ void __launch_bounds__(256) met_fixup_kernel(const FixupParams F) {
     }
 }
 
-// Final stage of a4: block k sums the tile partials of slot_at_rank[k] in fixed order and writes
-// the five observables by rank and by slot.
-__global__ void measure_finalize_kernel(const double* __restrict__ partials, int n_tiles,
-                                        const int* __restrict__ slot_at_rank,
-                                        double* __restrict__ obs_rank, double* __restrict__ obs_slot,
-                                        double* __restrict__ series_row) {
-    const int k = blockIdx.x;
-    const int slot = slot_at_rank[k];
-    __shared__ double red[3][32];
+// Final stage of a4, shared by the two kernels below: one WARP sums the tile partials of one slot in
+// fixed order (lane l takes tiles l, l+32, ..., then a shuffle tree) and lane 0 writes the five
+// observables by rank and by slot.
+__device__ __forceinline__ void finalize_rank(const double* __restrict__ partials, int n_tiles, int k, int slot, int lane,
+                                              double* __restrict__ obs_rank, double* __restrict__ obs_slot,
+                                              double* __restrict__ series_row) {
     double v[3] = { 0.0, 0.0, 0.0 };
-    for (int t = threadIdx.x; t < n_tiles; t += blockDim.x)
+    for (int t = lane; t < n_tiles; t += 32)
         for (int c = 0; c < 3; ++c) v[c] += partials[((size_t)slot * n_tiles + t) * 3 + c];
     for (int c = 0; c < 3; ++c)
         for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
-    const int wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    if ((threadIdx.x & 31) == 0) for (int c = 0; c < 3; ++c) red[c][wid] = v[c];
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double s[3] = { 0.0, 0.0, 0.0 };
-        for (int w = 0; w < nw; ++w) for (int c = 0; c < 3; ++c) s[c] += red[c][w];
-        const double m2 = s[1] * s[1] + s[2] * s[2];
-        const double o5[5] = { s[0], s[1], s[2], m2, m2 * m2 };
+    if (lane == 0) {
+        const double m2 = v[1] * v[1] + v[2] * v[2];
+        const double o5[5] = { v[0], v[1], v[2], m2, m2 * m2 };
         for (int c = 0; c < 5; ++c) {
             obs_rank[5 * k + c] = o5[c];
             obs_slot[5 * slot + c] = o5[c];
             if (series_row) series_row[5 * k + c] = o5[c];
         }
     }
+}
+
+// grid: one warp per rank
+__global__ void measure_finalize_kernel(const double* __restrict__ partials, int n_tiles, int R,
+                                        const int* __restrict__ slot_at_rank,
+                                        double* __restrict__ obs_rank, double* __restrict__ obs_slot,
+                                        double* __restrict__ series_row) {
+    const int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (k < R) finalize_rank(partials, n_tiles, k, slot_at_rank[k], threadIdx.x & 31, obs_rank, obs_slot, series_row);
 }
 
 // a5: one replica exchange (Eq. 3) in fp64; thread per candidate pair.
@@ -143,6 +144,34 @@ __global__ void pt_exchange_kernel(int R, uint32_t n_pt, PhiloxKeys keys, const 
         beta_of_slot[a] = betas[k + 1]; beta_of_slot[b] = betas[k];
         beta32_of_slot[a] = (float)betas[k + 1]; beta32_of_slot[b] = (float)betas[k];
         pt_acc[k] += 1ull;
+    }
+}
+
+// a4 final stage + a5 in one launch (the Monte Carlo step's tail): the 32 warps of one block reduce
+// the ranks w, w+32, ... exactly like measure_finalize_kernel, then the block decides the exchanges.
+__global__ void __launch_bounds__(1024) finalize_pt_kernel(const double* __restrict__ partials, int n_tiles, int R, uint32_t n_pt,
+                                                          PhiloxKeys keys, const double* __restrict__ betas,
+                                                          int* __restrict__ slot_at_rank, double* __restrict__ obs_rank,
+                                                          double* __restrict__ obs_slot, double* __restrict__ series_row,
+                                                          double* __restrict__ beta_of_slot, float* __restrict__ beta32_of_slot,
+                                                          unsigned long long* __restrict__ pt_acc) {
+    for (int k = threadIdx.x >> 5; k < R; k += 32)
+        finalize_rank(partials, n_tiles, k, slot_at_rank[k], threadIdx.x & 31, obs_rank, obs_slot, series_row);
+    __syncthreads();
+    for (int pair = threadIdx.x; ; pair += blockDim.x) {
+        const int k = (int)(n_pt & 1u) + 2 * pair;
+        if (k + 1 >= R) break;
+        const int a = slot_at_rank[k], b = slot_at_rank[k + 1];
+        uint32_t w[4];
+        philox4x32_10((uint32_t)k, 0u, n_pt, kStreamPT, keys, w);
+        const double u = (double)w[0] * (1.0 / 4294967296.0);
+        const double prob = exp((betas[k] - betas[k + 1]) * (obs_slot[5 * a] - obs_slot[5 * b]));
+        if (u < prob) {
+            slot_at_rank[k] = b; slot_at_rank[k + 1] = a;
+            beta_of_slot[a] = betas[k + 1]; beta_of_slot[b] = betas[k];
+            beta32_of_slot[a] = (float)betas[k + 1]; beta32_of_slot[b] = (float)betas[k];
+            pt_acc[k] += 1ull;
+        }
     }
 }
 
