@@ -98,7 +98,7 @@ class XYOracle:
         self.set_threads(threads)
 
     def __del__(self):
-        if getattr(self, "_h", None):
+        if getattr(self, "_h", None) and lib is not None:                # None during interpreter shutdown
             lib().xyo_destroy(self._h)
             self._h = None
 

@@ -120,7 +120,7 @@ class XY:
                    "xy_attach")
 
     def close(self):
-        if getattr(self, "_h", None):
+        if getattr(self, "_h", None) and load_library is not None:       # None during interpreter shutdown
             load_library().xy_destroy(self._h)
             self._h = None
 
