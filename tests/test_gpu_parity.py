@@ -463,6 +463,36 @@ def test_full_size_configs_sampled_slots(xy_mod, oracle_mod, idx, slots):
     print(cfg.name, "pt", P.check_pt(xy.get_perm(), ora.get_perm(), tr["pt_p"], tr["pt_u"]))
 
 
+# ---- pipeline hazards --------------------------------------------------------------------------
+@pytest.mark.parametrize("L,R", [(32, 3), (64, 2), (128, 1), (160, 1)])
+def test_free_run_is_reproducible_across_kernel_variants(xy_mod, L, R):
+    """compute-sanitizer is closed on this pool, so races in the TMA / mbarrier pipeline are hunted
+    this way: a hazard between the bulk copies, the staging and the updates would make a free run
+    differ from run to run or from tiling to tiling.  The site arithmetic does not depend on the tile
+    shape, and the compile-time-geometry kernel does the same operations in the same order as the
+    run-time-geometry one, so 6 MCS from the same seed must end in BITWISE identical states."""
+    betas = inputs.beta_ladder(0.4535, 0.4550, R)
+    ref = None
+    variants = [dict(), dict(), dict(generic=1), dict(tz=8), dict(generic=1, tz=L), dict(ty=8, tz=16)]
+    for v in variants:
+        xy = xy_mod.XY(L, R, betas, SEED)
+        if "generic" in v:
+            xy.set_option(xy_mod.XY_OPT_GENERIC_KERNEL, 1)
+        if "ty" in v:
+            xy.set_option(xy_mod.XY_OPT_TILE_Y, v["ty"])
+        if "tz" in v:
+            xy.set_option(xy_mod.XY_OPT_TILE_Z, v["tz"])
+        xy.init_random()
+        xy.mcs(6)
+        S, perm, obs = xy.get_state(), xy.get_perm(), xy.measure()
+        if ref is None:
+            ref = (S, perm, obs)
+            continue
+        assert np.array_equal(S.view(np.uint32), ref[0].view(np.uint32)), v
+        assert np.array_equal(perm, ref[1]), v
+        assert np.allclose(obs[:, :3], ref[2][:, :3], rtol=0, atol=1e-6 * 3 * L ** 3), v
+
+
 # ---- P7: long-run statistics ---------------------------------------------------------------------
 def _run_means(series, N):
     """series [T,R,5] (after the discarded head) -> time averages E/N [R] and Q2 = <M4>/<M2>^2 [R]."""
