@@ -25,6 +25,8 @@
 //                      brute-force bond loop in Python
 //   PT exchange        equal-beta forced swaps (known permutation), R=1 no-op,
 //                      <E> invariance with PT on/off
+//   stiffness sums     ordered and helical closed forms per axis, E = -(Cx+Cy+Cz), odd / even
+//                      under theta -> -theta, global-rotation invariance, brute-force bond loop in Python
 // Parity unpinned: nothing in this file.
 //
 // Build: g++ -O2 -std=c++17 -shared -fPIC -pthread xy_oracle.cpp -o libxy_oracle.so
@@ -188,6 +190,26 @@ void measure_slot(const Ctx& c, int r, double out[5]) {
     out[0] = E; out[1] = Mx; out[2] = My; out[3] = M2; out[4] = M2 * M2;   // Eq. 5 ingredients
 }
 
+// The six sums of one slot that the spin-stiffness estimator is made of [P:58-60 Eq. 6]: for each
+// lattice direction mu = x, y, z, over the N bonds (i, i+mu):
+//   C_mu = sum cos(theta_i - theta_{i+mu}),   S_mu = sum sin(theta_i - theta_{i+mu}).
+// Eq. 6 is then rho_s = 1/(3N) sum_mu [ <C_mu> - (1/T) <S_mu^2> ] (host arithmetic on the time series).
+void stiffness_slot(const Ctx& c, int r, double out[6]) {
+    const int L = c.L;
+    const float* th = c.theta.data() + (int64_t)r * c.N;
+    double C[3] = { 0.0, 0.0, 0.0 }, S[3] = { 0.0, 0.0, 0.0 };
+    for (int z = 0; z < L; ++z)
+      for (int y = 0; y < L; ++y)
+        for (int x = 0; x < L; ++x) {
+            const double t = (double)th[x + (int64_t)L * (y + (int64_t)L * z)];
+            const double tn[3] = { (double)th[wrap(x + 1, L) + (int64_t)L * (y + (int64_t)L * z)],
+                                   (double)th[x + (int64_t)L * (wrap(y + 1, L) + (int64_t)L * z)],
+                                   (double)th[x + (int64_t)L * (y + (int64_t)L * wrap(z + 1, L))] };
+            for (int mu = 0; mu < 3; ++mu) { C[mu] += std::cos(t - tn[mu]); S[mu] += std::sin(t - tn[mu]); }
+        }
+    for (int mu = 0; mu < 3; ++mu) { out[mu] = C[mu]; out[3 + mu] = S[mu]; }
+}
+
 template <class F>
 void for_active_slots(Ctx& c, F f) {
     const int n = (int)c.active.size();
@@ -330,6 +352,16 @@ int xyo_measure(xyo_ctx* h, double* out) {
     std::vector<double> by_slot(5 * (size_t)c.R, std::nan(""));
     xyo_measure_slots(h, by_slot.data());
     for (int k = 0; k < c.R; ++k) std::memcpy(out + 5 * (size_t)k, by_slot.data() + 5 * (size_t)c.slot_at_rank[k], 5 * sizeof(double));
+    return 0;
+}
+
+// out[R][6] = Cx, Cy, Cz, Sx, Sy, Sz (see stiffness_slot) indexed by RANK k.
+int xyo_measure_stiffness(xyo_ctx* h, double* out) {
+    if (!h || !out) return -1;
+    Ctx& c = h->c;
+    std::vector<double> by_slot(6 * (size_t)c.R, std::nan(""));
+    for_active_slots(c, [&](int r) { stiffness_slot(c, r, by_slot.data() + 6 * (size_t)r); });
+    for (int k = 0; k < c.R; ++k) std::memcpy(out + 6 * (size_t)k, by_slot.data() + 6 * (size_t)c.slot_at_rank[k], 6 * sizeof(double));
     return 0;
 }
 

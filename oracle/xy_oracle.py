@@ -57,6 +57,7 @@ def lib():
             "xyo_overrelax_sweep": (i32, [vp]),
             "xyo_measure_slots": (i32, [vp, pd]),
             "xyo_measure": (i32, [vp, pd]),
+            "xyo_measure_stiffness": (i32, [vp, pd]),
             "xyo_pt_exchange_with_E": (i32, [vp, pd]),
             "xyo_pt_exchange": (i32, [vp]),
         }
@@ -195,6 +196,12 @@ class XYOracle:
     def measure(self):
         out = np.empty((self.R, 5), dtype=np.float64)
         _chk(lib().xyo_measure(self._h, _p(out, C.c_double)), "measure")
+        return out
+
+    def measure_stiffness(self):
+        """[R, 6] = Cx, Cy, Cz, Sx, Sy, Sz by rank: the sums of cos / sin of the bond angle per direction (Eq. 6)."""
+        out = np.empty((self.R, 6), dtype=np.float64)
+        _chk(lib().xyo_measure_stiffness(self._h, _p(out, C.c_double)), "measure_stiffness")
         return out
 
     def measure_slots(self):

@@ -228,6 +228,54 @@ def test_O7_helical_state(oracle_mod, k):
         assert np.max(H.angle_diff(o.get_state(), s)) < 5e-6
 
 
+# ---- f1: the spin-stiffness sums of Eq. 6 ---------------------------------------------
+def test_stiffness_sums_closed_forms_and_symmetries(oracle_mod):
+    L, R = 8, 1
+    N = L ** 3
+    o = oracle_mod.XYOracle(L, R, [0.45], SEED)
+    # ordered: every bond angle is 0 -> C_mu = N, S_mu = 0 (rho_s = 1 at T = 0)
+    o.set_state(inputs.ordered_state(L, R, 1.234))
+    assert np.allclose(o.measure_stiffness()[0], [N, N, N, 0, 0, 0], atol=1e-9)
+    # helical theta = 2 pi k.r / L: theta_i - theta_{i+mu} = -2 pi k_mu / L on every bond, each axis separately
+    for k in ((1, 0, 0), (0, 2, 0), (0, 0, 3), (2, 1, 3)):
+        o.set_state(inputs.helical_state(L, R, k, phase=0.3))
+        want = [N * np.cos(2 * np.pi * kk / L) for kk in k] + [-N * np.sin(2 * np.pi * kk / L) for kk in k]
+        assert np.allclose(o.measure_stiffness()[0], want, atol=2e-6 * N), k
+    # a random state: E = -(Cx + Cy + Cz); theta -> -theta flips S and keeps C; a global rotation keeps both
+    s = inputs.uniform_state(L, R, 5).astype(np.float64)
+    o.set_state(s.astype(np.float32))
+    a = o.measure_stiffness()[0]
+    assert abs(a[:3].sum() + o.measure()[0, 0]) < 1e-9 * N
+    o.set_state(((-s) % (2 * np.pi)).astype(np.float32))
+    b = o.measure_stiffness()[0]
+    assert np.allclose(b[:3], a[:3], atol=3e-6 * N) and np.allclose(b[3:], -a[3:], atol=3e-6 * N)
+    o.set_state(((s + 0.777) % (2 * np.pi)).astype(np.float32))
+    c = o.measure_stiffness()[0]
+    assert np.allclose(c, a, atol=3e-6 * N)
+
+
+def test_stiffness_sums_match_brute_force_bond_loop(oracle_mod):
+    L, R = 4, 2
+    s = inputs.uniform_state(L, R, 23)
+    o = oracle_mod.XYOracle(L, R, [0.4, 0.5], SEED)
+    o.set_state(s)
+    o.set_perm(np.array([1, 0], dtype=np.int32))            # rows are reported by rank
+    got = o.measure_stiffness()
+    for k, r in enumerate((1, 0)):
+        t = s[r].astype(np.float64)                          # [z][y][x]
+        want = []
+        for fn in (np.cos, np.sin):
+            for axis in (2, 1, 0):                           # x, y, z
+                tot = 0.0
+                for z in range(L):
+                    for y in range(L):
+                        for x in range(L):
+                            n = [z, y, x]; n[axis] = (n[axis] + 1) % L
+                            tot += fn(t[z, y, x] - t[n[0], n[1], n[2]])
+                want.append(tot)
+        assert np.allclose(got[k], want, rtol=1e-12, atol=1e-10)
+
+
 def test_O8_staggered_state(oracle_mod):
     L, R = 6, 1
     o = oracle_mod.XYOracle(L, R, [0.45], SEED)
