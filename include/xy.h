@@ -143,6 +143,14 @@ int xy_overrelax_sweep(xy_ctx* ctx);
  * produced. */
 int xy_measure(xy_ctx* ctx, double* out);
 
+/* The six sums behind the spin-stiffness estimator [P:58-60 Eq. 6] of the current state,
+ * out[R][6] = Cx, Cy, Cz, Sx, Sy, Sz indexed by RANK k, with, over the N bonds (i, i+mu) of
+ * direction mu,  C_mu = sum cos(theta_i - theta_{i+mu}),  S_mu = sum sin(theta_i - theta_{i+mu}).
+ * Eq. 6 is rho_s = 1/(3N) sum_mu [ <C_mu> - beta <S_mu^2> ], host arithmetic on the time series;
+ * E = -(Cx + Cy + Cz).  fp32 bond terms, fp64 fixed-order accumulation; one pass over the spins
+ * (4 B per site).  out: host pointer, R*6 doubles, written after a stream synchronise. */
+int xy_measure_stiffness(xy_ctx* ctx, double* out);
+
 /* One replica exchange [P:45-50 Eq. 3; R8-R11]: for k = n_pt mod 2, k+2, ... with k+1 < R,
  * a = slot_at_rank[k], b = slot_at_rank[k+1], u = W[0] * 2^-32 with
  * W = Philox(counter = (k, 0, n_pt, 3)); accept iff u < exp((betas[k]-betas[k+1])*(E_a-E_b)),

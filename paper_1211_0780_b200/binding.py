@@ -35,6 +35,7 @@ SIGNATURES = {
     "xy_metropolis_sweep": (_i, [_vp]),
     "xy_overrelax_sweep": (_i, [_vp]),
     "xy_measure": (_i, [_vp, _vp]),
+    "xy_measure_stiffness": (_i, [_vp, _vp]),
     "xy_pt_exchange": (_i, [_vp]),
     "xy_mcs": (_i, [_vp, _i, _vp]),
     "xy_get_perm": (_i, [_vp, _pi]),
@@ -164,6 +165,12 @@ class XY:
 
     def overrelax_sweep(self):
         _check(_lib.xy_overrelax_sweep(self._h), "xy_overrelax_sweep")
+
+    def measure_stiffness(self):
+        """[R, 6] = Cx, Cy, Cz, Sx, Sy, Sz by rank: cos / sin of the bond angle summed per direction (Eq. 6)."""
+        out = np.empty((self.R, 6), dtype=np.float64)
+        _check(_lib.xy_measure_stiffness(self._h, out.ctypes.data), "xy_measure_stiffness")
+        return out
 
     def measure(self, to_host=True):
         """[R,5] doubles E, Mx, My, |M|^2, |M|^4 by rank; to_host=False only enqueues the reduction."""

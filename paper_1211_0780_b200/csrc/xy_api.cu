@@ -35,7 +35,7 @@ bool shape_ok(int L, int R) { return L >= 8 && L % 8 == 0 && L <= 1024 && R >= 1
 size_t max_tiles(int L) { return (size_t)(L / 2) * (size_t)(L / 2); }   // tiles_ok: TY >= 2 and TZ >= 2
 
 struct WsLayout {
-    size_t obs_rank, obs_slot, partials, betas, beta_of_slot, beta32, slot_at_rank, met_acc, pt_acc, exact, near_ctl, near_queue, stage, total;
+    size_t obs_rank, obs_slot, partials, partials6, obs6, betas, beta_of_slot, beta32, slot_at_rank, met_acc, pt_acc, exact, near_ctl, near_queue, stage, total;
     unsigned int near_cap;
 };
 WsLayout ws_layout(int L, int R) {
@@ -45,6 +45,8 @@ WsLayout ws_layout(int L, int R) {
     w.obs_rank = take((size_t)R * 5 * 8);
     w.obs_slot = take((size_t)R * 5 * 8);
     w.partials = take((size_t)R * max_tiles(L) * 3 * 8);
+    w.partials6 = take((size_t)R * max_tiles(L) * 6 * 8);
+    w.obs6 = take((size_t)R * 6 * 8);
     w.betas = take((size_t)R * 8);
     w.beta_of_slot = take((size_t)R * 8);
     w.beta32 = take((size_t)R * 4);
@@ -155,7 +157,7 @@ int launch_sweep_impl(xy_ctx* c, const SweepParams& P) {
     const int threads = (P.nItems + 31) / 32 * 32 + 32;          // compute warps + the auxiliary warp
     dim3 grid(P.nTY * P.nTZ, c->R);
     {
-        LaunchSpan span(c, MODE == MODE_MET ? XY_K_METROPOLIS : MODE == MODE_OR ? XY_K_OVERRELAX : XY_K_MEASURE);
+        LaunchSpan span(c, MODE == MODE_MET ? XY_K_METROPOLIS : MODE == MODE_OR ? XY_K_OVERRELAX : XY_K_MEASURE);   // MODE_STIFF counts as measure
         sweep_kernel<MODE, TRACE, FUSED, EXACT_INLINE, W4C, TYC><<<grid, threads, smem, c->stream>>>(P);
     }
     CK(cudaGetLastError());
@@ -476,6 +478,24 @@ static int pt_exchange_impl(xy_ctx* c, double* d_series_row) {
     ++c->n_pt;
     c->rank_valid = false;                     // the by-rank rows now belong to the previous labelling
     return XY_OK;
+}
+
+int xy_measure_stiffness(xy_ctx* c, double* out) {
+    if (int rc = need(c)) return rc;
+    if (!out) return fail(XY_ERR_INVALID_ARG, "xy_measure_stiffness: NULL pointer");
+    SweepParams P = base_params(c, 1);         // own = white, staged = black
+    P.partials = c->ws_ptr<double>(c->ws.partials6);
+    if (int rc = launch_sweep<MODE_STIFF, false, false>(c, P)) return rc;
+    const int n_tiles = (c->L / c->TY) * (c->L / c->TZ);
+    {
+        LaunchSpan span(c, XY_K_FINALIZE);
+        stiffness_finalize_kernel<<<(c->R + 3) / 4, 128, 0, c->stream>>>(c->ws_ptr<double>(c->ws.partials6), n_tiles, c->R,
+                                                                       c->ws_ptr<int>(c->ws.slot_at_rank),
+                                                                       c->ws_ptr<double>(c->ws.obs6));
+    }
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(out, c->ws_ptr<double>(c->ws.obs6), (size_t)c->R * 6 * 8, cudaMemcpyDeviceToHost, c->stream));
+    return check_near_overflow(c);
 }
 
 int xy_pt_exchange(xy_ctx* c) {

@@ -147,6 +147,21 @@ __global__ void pt_exchange_kernel(int R, uint32_t n_pt, PhiloxKeys keys, const 
     }
 }
 
+// Final stage of the six spin-stiffness sums: one warp per rank, fixed order.
+__global__ void stiffness_finalize_kernel(const double* __restrict__ partials6, int n_tiles, int R,
+                                          const int* __restrict__ slot_at_rank, double* __restrict__ out6_rank) {
+    const int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (k >= R) return;
+    const int slot = slot_at_rank[k];
+    double v[6] = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
+    for (int t = lane; t < n_tiles; t += 32)
+        for (int c = 0; c < 6; ++c) v[c] += partials6[((size_t)slot * n_tiles + t) * 6 + c];
+    for (int c = 0; c < 6; ++c)
+        for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
+    if (lane == 0)
+        for (int c = 0; c < 6; ++c) out6_rank[6 * k + c] = v[c];
+}
+
 // a4 final stage + a5 in one launch (the Monte Carlo step's tail): the 32 warps of one block reduce
 // the ranks w, w+32, ... exactly like measure_finalize_kernel, then the block decides the exchanges.
 __global__ void __launch_bounds__(1024) finalize_pt_kernel(const double* __restrict__ partials, int n_tiles, int R, uint32_t n_pt,

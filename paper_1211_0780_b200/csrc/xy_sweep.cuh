@@ -29,7 +29,7 @@
 
 namespace xyk {
 
-enum { MODE_MET = 0, MODE_OR = 1, MODE_MEASURE = 2 };
+enum { MODE_MET = 0, MODE_OR = 1, MODE_MEASURE = 2, MODE_STIFF = 3 };
 constexpr int kRing = 3;                 // staged (cos, sin) planes resident in shared memory
 constexpr int kRaw = 6;                  // raw-angle slots filled by bulk copies (a multiple of kRing: see the march)
 constexpr int kAhead = 3;                // steps between issuing a copy and reading its slot
@@ -48,7 +48,7 @@ struct SweepParams {
     unsigned long long* met_acc; // Metropolis: accepted proposals per slot
     unsigned long long* exact_count;  // Metropolis: decisions re-evaluated in fp64
     float* trace;                // Metropolis test hook: p_fast per own site (same layout as own) or null
-    double* partials;            // measure: [R][nTY*nTZ][3] partial E, Mx, My
+    double* partials;            // measure: [R][nTY*nTZ][3] partial E, Mx, My; MODE_STIFF: [R][nTY*nTZ][6] Cx,Cy,Cz,Sx,Sy,Sz
     uint4* near_queue;           // Metropolis: decisions too close to call in fp32 (see met_fixup_kernel)
     unsigned int* near_count;    // entries appended so far in this colour pass
     unsigned int near_cap;       // capacity of near_queue
@@ -186,6 +186,9 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
     __syncthreads();
 
     constexpr bool MEAS = (MODE == MODE_MEASURE) || FUSED;
+    constexpr bool STIFF = MODE == MODE_STIFF;          // the six bond sums of Eq. 6 instead of E, Mx, My
+    float acc6[6] = { 0.f, 0.f, 0.f, 0.f, 0.f, 0.f };
+    double d6[6] = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
     f32x2 accM = 0ull;                               // per-plane fp32 (Mx, My), flushed to double each plane
     float accE = 0.f;
     double dE = 0.0, dMx = 0.0, dMy = 0.0;
@@ -328,6 +331,28 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
                     const f32x2 e = lds_p1(aZ + (par ? eRel1 : eRel0));
                     const ulonglong2 aA = lds_p2(aZ - rowB), aB = lds_p2(aZ - rowB + partB);
                     const ulonglong2 bA = lds_p2(aZ + rowB), bB = lds_p2(aZ + rowB + partB);
+                    if (STIFF) {
+                        // Per direction mu and own (white) site i the two bonds (i-mu, i) and (i, i+mu):
+                        //   C_mu += S_i . (S_- + S_+),   S_mu += sin_i (cos_+ - cos_-) - cos_i (sin_+ - sin_-);
+                        // the white sites' bonds are all bonds (bipartite lattice).  Not a hot path: scalar fp32.
+                        const f32x2 ym[4] = { aA.x, aA.y, aB.x, aB.y }, yp[4] = { bA.x, bA.y, bB.x, bB.y };
+                        const float own4[4] = { cur.x, cur.y, cur.z, cur.w };
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            const f32x2 xm = par ? pc[k] : (k == 0 ? e : pc[k - 1]);
+                            const f32x2 xp = par ? (k == 3 ? e : pc[k + 1]) : pc[k];
+                            const f32x2 lo[3] = { xm, ym[k], pm[k] }, hi[3] = { xp, yp[k], pp[k] };
+                            float si, ci;
+                            fast_sincos(own4[k], si, ci);
+#pragma unroll
+                            for (int mu = 0; mu < 3; ++mu) {
+                                float cm, sm, cp, sp;
+                                unpack2(lo[mu], cm, sm); unpack2(hi[mu], cp, sp);
+                                acc6[mu] = fmaf(ci, cm + cp, fmaf(si, sm + sp, acc6[mu]));
+                                acc6[3 + mu] = fmaf(si, cp - cm, fmaf(-ci, sp - sm, acc6[3 + mu]));
+                            }
+                        }
+                    }
                     const f32x2 y0s = add2(add2(aA.x, bA.x), add2(pm[0], pp[0]));
                     const f32x2 y1s = add2(add2(aA.y, bA.y), add2(pm[1], pp[1]));
                     const f32x2 y2s = add2(add2(aB.x, bB.x), add2(pm[2], pp[2]));
@@ -407,7 +432,7 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
                             accM = add2(accM, pack2(cs, sn));
                         }
                     }
-                } else {  // MODE_MEASURE: own = white; E = -sum_white S_i . h_i counts every bond once
+                } else if (MODE == MODE_MEASURE) {  // own = white; E = -sum_white S_i . h_i counts every bond once
 #pragma unroll
                     for (int k = 0; k < 4; ++k) {
                         float hx, hy, sn, cs;
@@ -417,7 +442,11 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
                         accM = add2(accM, pack2(cs, sn));
                     }
                 }
-                if (MODE != MODE_MEASURE && active) *reinterpret_cast<float4*>(gp) = make_float4(th[0], th[1], th[2], th[3]);
+                if (MODE != MODE_MEASURE && !STIFF && active) *reinterpret_cast<float4*>(gp) = make_float4(th[0], th[1], th[2], th[3]);
+                if (STIFF) {
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) { if (active) d6[c] += (double)acc6[c]; acc6[c] = 0.f; }
+                }
                 if (MEAS) {
                     float mx, my;
                     unpack2(accM, mx, my);
@@ -457,21 +486,25 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 544, W4C ? XY_SWEEP_MIN
             if (e) atomicAdd(P.exact_count, (unsigned long long)e);
         }
     }
-    if (MEAS) {
+    if (MEAS || STIFF) {
         // fixed-order block reduction in double: warp shuffle tree, then warp 0 sums the warps in order
-        __shared__ double red[3][32];
-        double v[3] = { dE, dMx, dMy };
+        constexpr int NV = STIFF ? 6 : 3;
+        __shared__ double red[NV][32];
+        double v[6] = { STIFF ? d6[0] : dE, STIFF ? d6[1] : dMx, STIFF ? d6[2] : dMy, d6[3], d6[4], d6[5] };
 #pragma unroll
-        for (int c = 0; c < 3; ++c)
+        for (int c = 0; c < NV; ++c)
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
         const int wid = tid >> 5, nw = (blockDim.x + 31) >> 5;
-        if ((tid & 31) == 0) { red[0][wid] = v[0]; red[1][wid] = v[1]; red[2][wid] = v[2]; }
+        if ((tid & 31) == 0) {
+#pragma unroll
+            for (int c = 0; c < NV; ++c) red[c][wid] = v[c];
+        }
         __syncthreads();
-        if (tid < 3) {
+        if (tid < NV) {
             double sum = 0.0;
             for (int k = 0; k < nw; ++k) sum += red[tid][k];
-            P.partials[((size_t)slot * gridDim.x + tile) * 3 + tid] = tid == 0 ? -sum : sum;
+            P.partials[((size_t)slot * gridDim.x + tile) * NV + tid] = (!STIFF && tid == 0) ? -sum : sum;
         }
     }
 }

@@ -279,6 +279,33 @@ def test_measure_fused_into_overrelax(xy_mod, oracle_mod, L, R):
     P.check_observables(unfused, ora.measure(), L ** 3)
 
 
+@pytest.mark.parametrize("L,R", SHAPES + [(160, 1)])
+def test_stiffness_sums_against_oracle(xy_mod, oracle_mod, L, R):
+    """f1 (Eq. 6): the six per-direction bond sums, GPU vs oracle, by rank; fp32 bond terms
+    with the stated 7.5e-7 sin/cos error -> |delta| <= 4e-6 * N per sum; E = -(Cx+Cy+Cz)."""
+    xy, ora = make(xy_mod, oracle_mod, L, R)
+    N = L ** 3
+    if R >= 3:
+        perm = np.roll(np.arange(R, dtype=np.int32), 1)
+        xy.set_perm(perm); ora.set_perm(perm)
+    for name, S in states_for(L, R):
+        xy.set_state(S); ora.set_state(S)
+        g, o = xy.measure_stiffness(), ora.measure_stiffness()
+        assert np.all(np.abs(g - o) <= 4e-6 * N), (name, np.abs(g - o).max() / N)
+        assert np.all(np.abs(g[:, :3].sum(axis=1) + xy.measure()[:, 0]) <= 4e-6 * 3 * N)
+    # closed forms on the GPU: ordered (rho_s = 1 at T = 0) and helical, each axis separately
+    xy.set_state(inputs.ordered_state(L, R, 0.7))
+    assert np.all(np.abs(xy.measure_stiffness() - np.array([N, N, N, 0, 0, 0.0])) <= 4e-6 * N)
+    for k in ((1, 0, 0), (0, 2, 0), (0, 0, 3)):
+        xy.set_state(inputs.helical_state(L, R, k, phase=0.3))
+        want = np.array([N * np.cos(2 * np.pi * kk / L) for kk in k] + [-N * np.sin(2 * np.pi * kk / L) for kk in k])
+        assert np.all(np.abs(xy.measure_stiffness() - want) <= 4e-6 * N), k
+    # the call must leave the state and the cached observables alone
+    xy.set_state(S)
+    a = xy.measure(); xy.measure_stiffness()
+    assert np.array_equal(a, xy.measure()) and np.array_equal(xy.get_state().view(np.uint32), S.view(np.uint32))
+
+
 def test_measure_closed_forms(xy_mod):
     """O3 / O7 / O8 on the GPU reduction: ordered, helical (each axis separately) and staggered."""
     L, R = 16, 2
