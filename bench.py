@@ -166,6 +166,8 @@ def run_ours(args, cfg):
         xy.init_ordered(0.0)
     if args.tile_z:
         xy.set_option(binding.XY_OPT_TILE_Z, args.tile_z)
+    if args.generic_kernel:
+        xy.set_option(binding.XY_OPT_GENERIC_KERNEL, 1)
     def barrier():
         if world > 1:
             dist.barrier()
@@ -277,6 +279,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--tile-z", type=int, default=0, help="override the march length (tuning; 0 = library default)")
+    ap.add_argument("--generic-kernel", action="store_true", help="force the run-time-geometry colour-pass kernel (tuning)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     cfg = inputs.CONFIGS[args.config]

@@ -48,7 +48,7 @@ enum {
 
 /* Tunables for xy_set_option (all optional; defaults are chosen from L and R). */
 enum {
-    XY_OPT_TILE_Y = 1,     /* rows of one colour per thread block (must divide L, TILE_Y*L/8 <= 1024) */
+    XY_OPT_TILE_Y = 1,     /* rows of one colour per thread block (must divide L, TILE_Y*L/8 <= 352) */
     XY_OPT_TILE_Z = 2,     /* planes a thread block marches through (must divide L)                  */
     XY_OPT_TRACE = 3,      /* 1: xy_metropolis_sweep also records its fast-path acceptance probability
                               per site (test hook; allocates R*N floats inside the library)         */

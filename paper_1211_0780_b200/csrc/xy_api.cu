@@ -142,7 +142,7 @@ void default_tiles(int L, int R, int& TY, int& TZ) {
 }
 
 bool tiles_ok(int L, int TY, int TZ) {
-    return TY >= 2 && TZ >= 2 && L % TY == 0 && L % TZ == 0 && TY * (L / 8) <= 512 &&
+    return TY >= 2 && TZ >= 2 && L % TY == 0 && L % TZ == 0 && TY * (L / 8) <= 352 &&   // 11 compute warps + the auxiliary warp
            sweep_smem_bytes(L, TY) <= 200 * 1024;
 }
 
