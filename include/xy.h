@@ -57,8 +57,10 @@ enum {
                               after xy_overrelax_sweep read no spins; 0: always the standalone reduction */
     XY_OPT_PROFILE = 5,    /* 1: bracket every kernel launch with a CUDA-event pair on the attached
                               stream; xy_get_kernel_times returns the per-class device times         */
-    XY_OPT_GENERIC_KERNEL = 6 /* 1: always run the colour-pass kernel that reads the row geometry at run
+    XY_OPT_GENERIC_KERNEL = 6, /* 1: always run the colour-pass kernel that reads the row geometry at run
                               time, also for L = 32, 64, 128, 160 where a compile-time variant exists  */
+    XY_OPT_OR_PER_MCS = 7  /* over-relaxation sweeps per Monte Carlo step of xy_mcs (default 1, P:30;
+                              P:43 "after several sweeps": microcanonical sweeps are cheap decorrelation) */
 };
 
 /* Kernel classes reported by xy_get_kernel_times. */
@@ -158,7 +160,7 @@ int xy_measure_stiffness(xy_ctx* ctx, double* out);
  * energies, running the reduction first if they are stale.  ++n_pt. */
 int xy_pt_exchange(xy_ctx* ctx);
 
-/* n_mcs repetitions of (Metropolis sweep, over-relaxation sweep, measure, PT exchange) [P:30],
+/* n_mcs repetitions of (Metropolis sweep, XY_OPT_OR_PER_MCS over-relaxation sweeps, measure, PT exchange) [P:30],
  * enqueued without host synchronisation.  series: DEVICE pointer to n_mcs*R*5 doubles that
  * receives the by-rank observables of every step (measured before that step's exchange, R14),
  * or NULL. */

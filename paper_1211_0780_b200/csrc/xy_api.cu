@@ -83,7 +83,7 @@ struct xy_ctx {
     WsLayout ws;
     float* d_trace = nullptr;
     // options
-    int TY = 0, TZ = 0, trace = 0, fused = 1, generic = 0;
+    int TY = 0, TZ = 0, trace = 0, fused = 1, generic = 0, or_per_mcs = 1;
     // cache state
     bool partials_valid = false, rank_valid = false;
     uint64_t launches = 0;
@@ -424,18 +424,22 @@ int xy_metropolis_sweep(xy_ctx* c) {
     return XY_OK;
 }
 
-int xy_overrelax_sweep(xy_ctx* c) {
-    if (int rc = need(c)) return rc;
+static int overrelax_sweep_impl(xy_ctx* c, bool with_observables) {
     for (int colour = 0; colour < 2; ++colour) {
         SweepParams P = base_params(c, colour);
-        const bool fuse = c->fused && colour == 1;      // the white pass sees the final black sites
+        const bool fuse = with_observables && colour == 1;      // the white pass sees the final black sites
         int rc = fuse ? launch_sweep<MODE_OR, false, true>(c, P) : launch_sweep<MODE_OR, false, false>(c, P);
         if (rc) return rc;
     }
     ++c->n_or;
-    c->partials_valid = c->fused != 0;
+    c->partials_valid = with_observables;
     c->rank_valid = false;
     return XY_OK;
+}
+
+int xy_overrelax_sweep(xy_ctx* c) {
+    if (int rc = need(c)) return rc;
+    return overrelax_sweep_impl(c, c->fused != 0);
 }
 
 int xy_measure(xy_ctx* c, double* out) {
@@ -508,7 +512,8 @@ int xy_mcs(xy_ctx* c, int n_mcs, double* d_series) {
     if (n_mcs < 0) return fail(XY_ERR_INVALID_ARG, "xy_mcs: n_mcs < 0");
     for (int t = 0; t < n_mcs; ++t) {
         if (int rc = xy_metropolis_sweep(c)) return rc;
-        if (int rc = xy_overrelax_sweep(c)) return rc;
+        for (int j = 0; j < c->or_per_mcs; ++j)          // only the last sweep's white pass carries the observables
+            if (int rc = overrelax_sweep_impl(c, c->fused != 0 && j + 1 == c->or_per_mcs)) return rc;
         if (int rc = pt_exchange_impl(c, d_series ? d_series + (size_t)t * c->R * 5 : nullptr)) return rc;
     }
     return XY_OK;
@@ -581,6 +586,9 @@ int xy_set_option(xy_ctx* c, int option, int value) {
         case XY_OPT_FUSED_MEASURE: c->fused = value ? 1 : 0; return XY_OK;
         case XY_OPT_PROFILE: c->profile = value ? 1 : 0; return XY_OK;
         case XY_OPT_GENERIC_KERNEL: c->generic = value ? 1 : 0; return XY_OK;
+        case XY_OPT_OR_PER_MCS:
+            if (value < 0 || value > 1000) return fail(XY_ERR_INVALID_ARG, "XY_OPT_OR_PER_MCS=%d out of range", value);
+            c->or_per_mcs = value; return XY_OK;
         default: return fail(XY_ERR_INVALID_ARG, "unknown option %d", option);
     }
 }
@@ -594,6 +602,7 @@ int xy_get_option(xy_ctx* c, int option, int* value) {
         case XY_OPT_FUSED_MEASURE: *value = c->fused; return XY_OK;
         case XY_OPT_PROFILE: *value = c->profile; return XY_OK;
         case XY_OPT_GENERIC_KERNEL: *value = c->generic; return XY_OK;
+        case XY_OPT_OR_PER_MCS: *value = c->or_per_mcs; return XY_OK;
         default: return fail(XY_ERR_INVALID_ARG, "unknown option %d", option);
     }
 }

@@ -520,6 +520,30 @@ def test_free_run_is_reproducible_across_kernel_variants(xy_mod, L, R):
         assert np.allclose(obs[:, :3], ref[2][:, :3], rtol=0, atol=1e-6 * 3 * L ** 3), v
 
 
+def test_mcs_with_several_overrelaxation_sweeps(xy_mod):
+    """XY_OPT_OR_PER_MCS: xy_mcs must equal the same calls made one by one, bit for bit, and its
+    series rows must be the observables of the state the last over-relaxation sweep left behind."""
+    import torch
+    L, R, n = 32, 4, 3
+    betas = inputs.beta_ladder(0.45, 0.46, R)
+    a, b = xy_mod.XY(L, R, betas, SEED), xy_mod.XY(L, R, betas, SEED)
+    a.init_random(); b.init_random()
+    a.set_option(xy_mod.XY_OPT_OR_PER_MCS, 3)
+    series = torch.zeros(n, R, 5, dtype=torch.float64, device="cuda")
+    a.mcs(n, series)
+    rows = []
+    for _ in range(n):
+        b.metropolis_sweep()
+        for _ in range(3):
+            b.overrelax_sweep()
+        rows.append(b.measure())
+        b.pt_exchange()
+    assert np.array_equal(a.get_state().view(np.uint32), b.get_state().view(np.uint32))
+    assert np.array_equal(a.get_perm(), b.get_perm())
+    assert np.array_equal(a.get_counters(), [n, 3 * n, n])
+    assert np.array_equal(series.cpu().numpy(), np.stack(rows))
+
+
 # ---- P7: long-run statistics ---------------------------------------------------------------------
 def _run_means(series, N):
     """series [T,R,5] (after the discarded head) -> time averages E/N [R] and Q2 = <M4>/<M2>^2 [R]."""
