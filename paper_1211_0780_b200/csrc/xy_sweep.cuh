@@ -60,6 +60,7 @@ typedef unsigned long long f32x2;
 __device__ __forceinline__ f32x2 pack2(float lo, float hi) { f32x2 d; asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi)); return d; }
 __device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
 __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
 // y + (par ? x1 : x0) as two predicated packed additions (one executes): no 64-bit selects
 __device__ __forceinline__ f32x2 add2_sel(f32x2 y, f32x2 x0, f32x2 x1, int par) {
     f32x2 d;
@@ -190,7 +191,7 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 384, XY_SWEEP_MIN_BLOCK
     float acc6[6] = { 0.f, 0.f, 0.f, 0.f, 0.f, 0.f };
     double d6[6] = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
     f32x2 accM = 0ull;                               // per-plane fp32 (Mx, My), flushed to double each plane
-    float accE = 0.f;
+    f32x2 accE = 0ull;                               // (sum cos_i h_x, sum sin_i h_y): E = -(x + y)
     double dE = 0.0, dMx = 0.0, dMy = 0.0;
     unsigned int nacc = 0, nexact = 0;
     bool active = false;
@@ -428,18 +429,19 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 384, XY_SWEEP_MIN_BLOCK
                         if (FUSED) {                                            // observables of the NEW state
                             float sn, cs;
                             fast_sincos(th[k], sn, cs);
-                            accE = fmaf(cs, hx, fmaf(sn, hy, accE));
-                            accM = add2(accM, pack2(cs, sn));
+                            const f32x2 sp = pack2(cs, sn);
+                            accE = fma2(sp, h[k], accE);
+                            accM = add2(accM, sp);
                         }
                     }
                 } else if (MODE == MODE_MEASURE) {  // own = white; E = -sum_white S_i . h_i counts every bond once
 #pragma unroll
                     for (int k = 0; k < 4; ++k) {
-                        float hx, hy, sn, cs;
-                        unpack2(h[k], hx, hy);
+                        float sn, cs;
                         fast_sincos(th[k], sn, cs);
-                        accE = fmaf(cs, hx, fmaf(sn, hy, accE));
-                        accM = add2(accM, pack2(cs, sn));
+                        const f32x2 sp = pack2(cs, sn);
+                        accE = fma2(sp, h[k], accE);
+                        accM = add2(accM, sp);
                     }
                 }
                 if (MODE != MODE_MEASURE && !STIFF && active) *reinterpret_cast<float4*>(gp) = make_float4(th[0], th[1], th[2], th[3]);
@@ -448,10 +450,11 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 384, XY_SWEEP_MIN_BLOCK
                     for (int c = 0; c < 6; ++c) { if (active) d6[c] += (double)acc6[c]; acc6[c] = 0.f; }
                 }
                 if (MEAS) {
-                    float mx, my;
+                    float mx, my, ex, ey;
                     unpack2(accM, mx, my);
-                    if (active) { dE += (double)accE; dMx += (double)mx; dMy += (double)my; }
-                    accE = 0.f; accM = 0ull;
+                    unpack2(accE, ex, ey);
+                    if (active) { dE += (double)(ex + ey); dMx += (double)mx; dMy += (double)my; }
+                    accE = 0ull; accM = 0ull;
                 }
                 gz += planeG;
                 gp += planeG;
