@@ -174,7 +174,8 @@ __device__ __noinline__ bool metropolis_exact(const float* __restrict__ other, i
 // path's g = h.(S' - S) is off by at most |dh||dS| + |h||d(dS)| <= 6 e_s * 2 sqrt2 + 2 e_s * 6 sqrt2
 // = 34 e_s = 2.6e-5 plus fp32 rounding of the six-term sums and the two products (< 8e-6), so
 // |p_fast - p| <= p beta |dg| < beta * 3.4e-5 for p <= 1; ex2.approx and the rounding of its argument
-// add < 1e-6 relative.  kWindowPerBeta = 4e-5 and kWindowAbs = 1.5e-6 leave a margin on both.
+// add < 1e-6 relative; the fast path compares against fl32(word) * 2^-32, which is u24 up to 2^-24 = 6e-8.
+// kWindowPerBeta = 4e-5 and kWindowAbs = 1.5e-6 leave a margin on all of these.
 // tests/test_gpu_parity.py::test_fast_path_window measures the actual |p_fast - p_oracle|.
 constexpr float kWindowPerBeta = 4.0e-5f;
 constexpr float kWindowAbs = 1.5e-6f;

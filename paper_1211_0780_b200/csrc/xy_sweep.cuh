@@ -301,7 +301,7 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 384, XY_SWEEP_MIN_BLOCK
         if (MODE == MODE_MET) {
             beta32 = P.beta32_of_slot[slot];
             bl = beta32 * 1.44269504f;               // exp(beta g) = 2^(bl g)
-            win24 = (fabsf(beta32) * kWindowPerBeta + kWindowAbs) * 16777216.0f;    // see xy_device.cuh
+            win24 = (fabsf(beta32) * kWindowPerBeta + kWindowAbs) * 4294967296.0f;  // window in units of 2^-32, see xy_device.cuh
             inv = philox_block_invariants((uint32_t)slot, P.sweep, P.colour == 0 ? kStreamMetBlack : kStreamMetWhite, P.keys);
             keep(bl); keep(win24); keep(inv.j0); keep(inv.j1); keep(inv.j2); keep(inv.j3);
         }
@@ -382,20 +382,22 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 384, XY_SWEEP_MIN_BLOCK
                             const int k = 2 * pr + kk;
                             const float kf = (float)(w[2 * kk] >> 8);
                             const float tn = kf * kTwoPiU24;
-                            const float uf = (float)(w[2 * kk + 1] >> 8);        // u24 * 2^24
+                            // acceptance uniform, fast path: the whole word converted in ONE instruction (2^32 u24 up
+                            // to the rounding of its low byte, < 2^-24 absolute, which kWindowAbs covers)
+                            const float uf = (float)w[2 * kk + 1];
                             float hx, hy, so, co, sn, cn;
                             unpack2(h[k], hx, hy);
                             fast_sincos(th[k], so, co);
                             fast_sincos(tn, sn, cn);
                             const float g = fmaf(hx, cn - co, hy * (sn - so));   // = -dE
-                            const float pf = fast_ex2(fmaf(bl, g, 24.0f));        // p * 2^24
+                            const float pf = fast_ex2(fmaf(bl, g, 32.0f));        // p * 2^32
                             bool acc = uf < pf;
                             dist[k] = fabsf(uf - pf);
                             if (EXACT_INLINE && dist[k] < win24) {
-                                acc = metropolis_exact(other, L, W, par, 4 * q + k, y, z0 + s - 2, th[k], tn, uf * kInvU24, beta32);
+                                acc = metropolis_exact(other, L, W, par, 4 * q + k, y, z0 + s - 2, th[k], tn, word_to_u24(w[2 * kk + 1]), beta32);
                                 ++nexact;
                             }
-                            if (TRACE) ptrace[k] = fminf(pf * kInvU24, 3.0e38f);
+                            if (TRACE) ptrace[k] = fminf(pf * 2.3283064365386963e-10f, 3.0e38f);
                             if (acc) { th[k] = tn; ++nacc; }
                         }
                     }

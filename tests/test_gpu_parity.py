@@ -127,6 +127,40 @@ def test_device_math_errors(xy_mod):
         assert abs(got - want) <= 6e-7
 
 
+@pytest.mark.parametrize("L,R,beta_hi", [(32, 4, 0.47), (16, 3, 1.5)])
+def test_fast_path_window(xy_mod, oracle_mod, L, R, beta_hi):
+    """The fp32 fast path of the Metropolis decision may only be trusted outside the window
+    |u - p_fast| >= |beta| * 4e-5 + 1.5e-6 (xy_device.cuh): measure |p_fast - p_oracle| on every site
+    (XY_OPT_TRACE records p_fast) and require it to stay inside that window, with its u-rounding of
+    2^-24, wherever p <= 1 could decide anything."""
+    betas = inputs.beta_ladder(0.44, beta_hi, R)
+    xy, ora = make(xy_mod, oracle_mod, L, R, betas=betas)
+    xy.set_option(xy_mod.XY_OPT_TRACE, 1)
+    col = H.colour_mask(L)
+    for name, S in states_for(L, R):
+        xy.set_state(S); xy.set_counters([5, 0, 0])
+        ora.set_counters([5, 0, 0])
+        xy.metropolis_sweep()
+        pf = xy.debug_get_trace().astype(np.float64)
+        G = xy.get_state()
+        start = S
+        worst = 0.0
+        for c in (0, 1):
+            ora.set_state(start)
+            tr = ora.enable_trace(met=True)
+            ora.metropolis_pass(c)
+            sel = np.broadcast_to(col == c, S.shape)
+            p = tr["met_p"][sel]
+            d = np.abs(np.minimum(pf[sel], 1.0) - np.minimum(p, 1.0))           # only p <= 1 can change a decision
+            window = (np.abs(betas.astype(np.float32)).astype(np.float64) * 4e-5 + 1.5e-6)[:, None]
+            ratio = (d.reshape(R, -1) + 2.0 ** -24) / window
+            worst = max(worst, float(ratio.max()))
+            start = np.where(col[None] == 0, G, S)
+        ora.enable_trace()
+        print(L, R, name, "max (|p_fast - p| + 2^-24) / window =", worst)
+        assert worst < 0.5, "the fast path's error must stay well inside the re-evaluation window"
+
+
 # ---- a0 -------------------------------------------------------------------------------------
 @pytest.mark.parametrize("L,R", [(8, 8), (24, 3), (32, 4)])
 def test_init_random_is_bit_exact(xy_mod, oracle_mod, L, R):
