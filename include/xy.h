@@ -59,8 +59,10 @@ enum {
                               stream; xy_get_kernel_times returns the per-class device times         */
     XY_OPT_GENERIC_KERNEL = 6, /* 1: always run the colour-pass kernel that reads the row geometry at run
                               time, also for L = 32, 64, 128, 160 where a compile-time variant exists  */
-    XY_OPT_OR_PER_MCS = 7  /* over-relaxation sweeps per Monte Carlo step of xy_mcs (default 1, P:30;
+    XY_OPT_OR_PER_MCS = 7, /* over-relaxation sweeps per Monte Carlo step of xy_mcs (default 1, P:30;
                               P:43 "after several sweeps": microcanonical sweeps are cheap decorrelation) */
+    XY_OPT_CUDA_GRAPH = 8  /* 1 (default): xy_mcs replays one captured CUDA graph per step from its second
+                              step on (counters live on the device); 0: every kernel is launched eagerly  */
 };
 
 /* Kernel classes reported by xy_get_kernel_times. */
@@ -97,7 +99,8 @@ size_t xy_workspace_bytes(int L, int R);
 /* Binds device memory and a stream.  d_state / d_workspace: DEVICE pointers, 256-byte aligned,
  * of at least xy_state_bytes / xy_workspace_bytes, owned by the caller (PyTorch) and required to
  * outlive the context; either may be NULL, in which case the library cudaMallocs and owns it.
- * cuda_stream: a cudaStream_t (NULL = the legacy default stream).  Uploads the beta labels and
+ * cuda_stream: a cudaStream_t; NULL = the library creates a blocking stream of its own, which is
+ * implicitly ordered with the legacy default stream (that one cannot be captured into a CUDA graph).  Uploads the beta labels and
  * the identity permutation; the spin state is undefined until xy_init_* or xy_set_state. */
 int xy_attach(xy_ctx* ctx, void* d_state, void* d_workspace, void* cuda_stream);
 

@@ -35,7 +35,7 @@ bool shape_ok(int L, int R) { return L >= 8 && L % 8 == 0 && L <= 1024 && R >= 1
 size_t max_tiles(int L) { return (size_t)(L / 2) * (size_t)(L / 2); }   // tiles_ok: TY >= 2 and TZ >= 2
 
 struct WsLayout {
-    size_t obs_rank, obs_slot, partials, partials6, obs6, betas, beta_of_slot, beta32, slot_at_rank, met_acc, pt_acc, exact, near_ctl, near_queue, stage, total;
+    size_t obs_rank, obs_slot, partials, partials6, obs6, dctr, betas, beta_of_slot, beta32, slot_at_rank, met_acc, pt_acc, exact, near_ctl, near_queue, stage, total;
     unsigned int near_cap;
 };
 WsLayout ws_layout(int L, int R) {
@@ -47,6 +47,7 @@ WsLayout ws_layout(int L, int R) {
     w.partials = take((size_t)R * max_tiles(L) * 3 * 8);
     w.partials6 = take((size_t)R * max_tiles(L) * 6 * 8);
     w.obs6 = take((size_t)R * 6 * 8);
+    w.dctr = take(sizeof(DeviceCounters));
     w.betas = take((size_t)R * 8);
     w.beta_of_slot = take((size_t)R * 8);
     w.beta32 = take((size_t)R * 4);
@@ -79,11 +80,15 @@ struct xy_ctx {
     bool attached = false;
     float* d_state = nullptr; bool own_state = false;
     char* d_ws = nullptr; bool own_ws = false;
-    cudaStream_t stream = nullptr;
+    cudaStream_t stream = nullptr; bool own_stream = false;
     WsLayout ws;
     float* d_trace = nullptr;
     // options
-    int TY = 0, TZ = 0, trace = 0, fused = 1, generic = 0, or_per_mcs = 1;
+    int TY = 0, TZ = 0, trace = 0, fused = 1, generic = 0, or_per_mcs = 1, use_graph = 1;
+    // CUDA graph of one Monte Carlo step in device-counter mode (xy_mcs), rebuilt when graph_key changes
+    cudaGraphExec_t graph_exec = nullptr;
+    uint64_t graph_key = 0, graph_launches = 0;
+    bool device_counters = false;              // true while a step is being enqueued for capture
     // cache state
     bool partials_valid = false, rank_valid = false;
     uint64_t launches = 0;
@@ -206,6 +211,7 @@ SweepParams base_params(xy_ctx* c, int colour) {
     P.near_queue = c->ws_ptr<uint4>(c->ws.near_queue);
     P.near_count = c->ws_ptr<unsigned int>(c->ws.near_ctl);
     P.near_cap = c->ws.near_cap;
+    P.d_counters = c->device_counters ? c->ws_ptr<uint32_t>(c->ws.dctr) : nullptr;
     return P;
 }
 
@@ -296,6 +302,8 @@ void xy_destroy(xy_ctx* c) {
     if (c->d_trace) cudaFree(c->d_trace);
     for (auto& s : c->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
     for (auto e : c->free_events) cudaEventDestroy(e);
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
     delete c;
 }
 
@@ -317,6 +325,10 @@ int xy_attach(xy_ctx* c, void* d_state, void* d_workspace, void* cuda_stream) {
     if (prop.major < 10) return fail(XY_ERR_NO_DEVICE, "xy_attach: device %s is sm_%d%d; built for sm_100a only", prop.name, prop.major, prop.minor);
     if (((uintptr_t)d_state | (uintptr_t)d_workspace) & 255u) return fail(XY_ERR_INVALID_ARG, "xy_attach: buffers must be 256-byte aligned");
     c->stream = (cudaStream_t)cuda_stream;
+    if (!c->stream) {                          // the legacy default stream cannot be captured into a graph: use a
+        CK(cudaStreamCreate(&c->stream));      // BLOCKING stream of our own, which stays ordered with it
+        c->own_stream = true;
+    }
     if (d_state) { c->d_state = (float*)d_state; c->own_state = false; }
     else { CK(cudaMalloc(&c->d_state, xy_state_bytes(c->L, c->R))); c->own_state = true; }
     if (d_workspace) { c->d_ws = (char*)d_workspace; c->own_ws = false; }
@@ -408,7 +420,7 @@ int xy_metropolis_sweep(xy_ctx* c) {
             FixupParams F;
             memset(&F, 0, sizeof(F));
             F.own = P.own; F.other = P.other; F.L = c->L; F.W = c->L / 2; F.colour = colour; F.R = c->R;
-            F.half_n = P.half_n; F.keys = c->keys; F.sweep = c->n_met; F.beta32_of_slot = P.beta32_of_slot;
+            F.half_n = P.half_n; F.keys = c->keys; F.sweep = c->n_met; F.d_counters = P.d_counters; F.beta32_of_slot = P.beta32_of_slot;
             F.met_acc = P.met_acc; F.exact_count = P.exact_count; F.near_queue = P.near_queue;
             F.near_count = P.near_count; F.near_cap = P.near_cap;
             F.done_ticket = P.near_count + 1; F.overflow_flag = P.near_count + 2;
@@ -462,14 +474,15 @@ static int pt_exchange_impl(xy_ctx* c, double* d_series_row) {
         c->partials_valid = true;
         c->rank_valid = false;
     }
-    if (!c->rank_valid || d_series_row) {
+    if (!c->rank_valid || d_series_row || c->device_counters) {
         const int n_tiles = (c->L / c->TY) * (c->L / c->TZ);
         LaunchSpan span(c, XY_K_PT);
         finalize_pt_kernel<<<1, 1024, 0, c->stream>>>(
             c->ws_ptr<double>(c->ws.partials), n_tiles, c->R, c->n_pt, c->keys, c->ws_ptr<double>(c->ws.betas),
             c->ws_ptr<int>(c->ws.slot_at_rank), c->ws_ptr<double>(c->ws.obs_rank), c->ws_ptr<double>(c->ws.obs_slot),
             d_series_row, c->ws_ptr<double>(c->ws.beta_of_slot), c->ws_ptr<float>(c->ws.beta32),
-            c->ws_ptr<unsigned long long>(c->ws.pt_acc));
+            c->ws_ptr<unsigned long long>(c->ws.pt_acc),
+            c->device_counters ? c->ws_ptr<DeviceCounters>(c->ws.dctr) : nullptr, c->or_per_mcs);
     } else {
         const int pairs = c->R / 2 + 1;
         LaunchSpan span(c, XY_K_PT);
@@ -507,15 +520,65 @@ int xy_pt_exchange(xy_ctx* c) {
     return pt_exchange_impl(c, nullptr);
 }
 
+// One Monte Carlo step enqueued on the stream [P:30].
+static int enqueue_mcs(xy_ctx* c, double* d_series_row) {
+    if (int rc = xy_metropolis_sweep(c)) return rc;
+    for (int j = 0; j < c->or_per_mcs; ++j)          // only the last sweep's white pass carries the observables
+        if (int rc = overrelax_sweep_impl(c, c->fused != 0 && j + 1 == c->or_per_mcs)) return rc;
+    return pt_exchange_impl(c, d_series_row);
+}
+
+// Captures one step in device-counter mode (the kernels read n_met / n_pt / the series row from the
+// workspace and finalize_pt_kernel advances them), so that the same graph can be replayed.
+static int build_step_graph(xy_ctx* c, uint64_t key) {
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    const uint32_t n0[3] = { c->n_met, c->n_or, c->n_pt };
+    const uint64_t launches0 = c->launches;
+    cudaGraph_t graph = nullptr;
+    CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+    c->device_counters = true;
+    const int rc = enqueue_mcs(c, nullptr);
+    c->device_counters = false;
+    const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    c->n_met = n0[0]; c->n_or = n0[1]; c->n_pt = n0[2];      // nothing ran: the capture only recorded
+    c->graph_launches = c->launches - launches0;             // kernel nodes per step
+    c->launches = launches0;
+    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) return fail(XY_ERR_CUDA, "cudaStreamEndCapture failed: %s", cudaGetErrorString(e));
+    const cudaError_t e2 = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e2 != cudaSuccess) { c->graph_exec = nullptr; return fail(XY_ERR_CUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e2)); }
+    c->graph_key = key;
+    return XY_OK;
+}
+
 int xy_mcs(xy_ctx* c, int n_mcs, double* d_series) {
     if (int rc = need(c)) return rc;
     if (n_mcs < 0) return fail(XY_ERR_INVALID_ARG, "xy_mcs: n_mcs < 0");
-    for (int t = 0; t < n_mcs; ++t) {
-        if (int rc = xy_metropolis_sweep(c)) return rc;
-        for (int j = 0; j < c->or_per_mcs; ++j)          // only the last sweep's white pass carries the observables
-            if (int rc = overrelax_sweep_impl(c, c->fused != 0 && j + 1 == c->or_per_mcs)) return rc;
-        if (int rc = pt_exchange_impl(c, d_series ? d_series + (size_t)t * c->R * 5 : nullptr)) return rc;
+    int t = 0;
+    // XY_OPT_CUDA_GRAPH: from the second step on, replay one captured graph per step (7 kernel nodes):
+    // same kernels, same arithmetic, less launch latency.  The first step runs eagerly (it also sets the
+    // kernels' attributes).  Profiling brackets launches with events and the test trace allocates: eager.
+    if (c->use_graph && !c->profile && !c->trace && n_mcs >= 3) {
+        if (int rc = enqueue_mcs(c, d_series)) return rc;
+        t = 1;
+        const uint64_t key = 1u | ((uint64_t)c->TY << 1) ^ ((uint64_t)c->TZ << 12) ^ ((uint64_t)c->fused << 23) ^ ((uint64_t)c->generic << 24) ^
+                             ((uint64_t)c->or_per_mcs << 25) ^ ((uint64_t)need_inline_exact(c) << 36) ^ ((uint64_t)(uintptr_t)c->stream << 37);
+        if (!c->graph_exec || c->graph_key != key)
+            if (int rc = build_step_graph(c, key)) return rc;
+        DeviceCounters v;
+        v.n_met = c->n_met; v.n_or = c->n_or; v.n_pt = c->n_pt; v.row = 1u; v.series_base = d_series;
+        set_device_counters_kernel<<<1, 1, 0, c->stream>>>(c->ws_ptr<DeviceCounters>(c->ws.dctr), v);
+        CK(cudaGetLastError());
+        for (; t < n_mcs; ++t) CK(cudaGraphLaunch(c->graph_exec, c->stream));
+        c->n_met += (uint32_t)(n_mcs - 1); c->n_or += (uint32_t)(n_mcs - 1) * (uint32_t)c->or_per_mcs; c->n_pt += (uint32_t)(n_mcs - 1);
+        c->launches += c->graph_launches * (uint64_t)(n_mcs - 1) + 1;
+        c->partials_valid = true;                  // the step's exchange reduced the final state (labels move, spins do not)
+        c->rank_valid = false;
+        return XY_OK;
     }
+    for (; t < n_mcs; ++t)
+        if (int rc = enqueue_mcs(c, d_series ? d_series + (size_t)t * c->R * 5 : nullptr)) return rc;
     return XY_OK;
 }
 
@@ -586,6 +649,7 @@ int xy_set_option(xy_ctx* c, int option, int value) {
         case XY_OPT_FUSED_MEASURE: c->fused = value ? 1 : 0; return XY_OK;
         case XY_OPT_PROFILE: c->profile = value ? 1 : 0; return XY_OK;
         case XY_OPT_GENERIC_KERNEL: c->generic = value ? 1 : 0; return XY_OK;
+        case XY_OPT_CUDA_GRAPH: c->use_graph = value ? 1 : 0; return XY_OK;
         case XY_OPT_OR_PER_MCS:
             if (value < 0 || value > 1000) return fail(XY_ERR_INVALID_ARG, "XY_OPT_OR_PER_MCS=%d out of range", value);
             c->or_per_mcs = value; return XY_OK;
@@ -603,6 +667,7 @@ int xy_get_option(xy_ctx* c, int option, int* value) {
         case XY_OPT_PROFILE: *value = c->profile; return XY_OK;
         case XY_OPT_GENERIC_KERNEL: *value = c->generic; return XY_OK;
         case XY_OPT_OR_PER_MCS: *value = c->or_per_mcs; return XY_OK;
+        case XY_OPT_CUDA_GRAPH: *value = c->use_graph; return XY_OK;
         default: return fail(XY_ERR_INVALID_ARG, "unknown option %d", option);
     }
 }

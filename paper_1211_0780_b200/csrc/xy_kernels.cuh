@@ -11,12 +11,20 @@ namespace xyk {
 // window of xy_device.cuh): the definition of include/xy.h in fp64 from the STORED angles.  Runs
 // after each colour pass, before anything reads the updated colour.  Eight lanes share an entry
 // (six neighbours, old angle, proposal: one fp64 sincos each).
+// Counters of a Monte Carlo step kept on the device so that ONE captured CUDA graph of a step can be
+// replayed: the Metropolis kernels read n_met, finalize_pt_kernel reads n_pt and the series row and
+// advances everything at the end of the step.
+struct DeviceCounters { uint32_t n_met, n_or, n_pt, row; double* series_base; };
+
+__global__ void set_device_counters_kernel(DeviceCounters* dc, DeviceCounters v) { *dc = v; }
+
 struct FixupParams {
     float* own; const float* other;
     int L, W, colour, R;
     unsigned int half_n;
     PhiloxKeys keys;
     uint32_t sweep;
+    const uint32_t* d_counters;      // when not null: sweep = d_counters[0] (CUDA-graph replay)
     const float* beta32_of_slot;
     unsigned long long* met_acc;
     unsigned long long* exact_count;
@@ -35,6 +43,7 @@ __global__ void __launch_bounds__(256) met_fixup_kernel(const FixupParams F) {
     const int lane = threadIdx.x & 31, role = lane & 7;
     const unsigned int groups = (gridDim.x * blockDim.x) >> 3;
     const uint32_t stream = F.colour == 0 ? kStreamMetBlack : kStreamMetWhite;
+    const uint32_t sweep = F.d_counters ? F.d_counters[0] : F.sweep;
     for (unsigned int e0 = ((blockIdx.x * blockDim.x + threadIdx.x) >> 5) << 2; e0 < n; e0 += groups) {   // warp-uniform trip count
         const unsigned int e = e0 + (lane >> 3);
         const bool live = e < n;
@@ -49,7 +58,7 @@ __global__ void __launch_bounds__(256) met_fixup_kernel(const FixupParams F) {
         const int par = (y + z + F.colour) & 1;                     // x parity of this site
         const uint32_t i = (uint32_t)(2 * xh + par) + (uint32_t)L * (uint32_t)(y + L * z);
         uint32_t w[4];
-        philox4x32_10(i >> 2, (uint32_t)slot, F.sweep, stream, F.keys, w);
+        philox4x32_10(i >> 2, (uint32_t)slot, sweep, stream, F.keys, w);
         const int p = (int)((i >> 1) & 1u);
         const float t_new = word_to_angle(p ? w[2] : w[0]);
         const float u = word_to_u24(p ? w[3] : w[1]);
@@ -169,7 +178,12 @@ __global__ void __launch_bounds__(1024) finalize_pt_kernel(const double* __restr
                                                           int* __restrict__ slot_at_rank, double* __restrict__ obs_rank,
                                                           double* __restrict__ obs_slot, double* __restrict__ series_row,
                                                           double* __restrict__ beta_of_slot, float* __restrict__ beta32_of_slot,
-                                                          unsigned long long* __restrict__ pt_acc) {
+                                                          unsigned long long* __restrict__ pt_acc, DeviceCounters* __restrict__ dc,
+                                                          int or_per_mcs) {
+    if (dc) {                                    // CUDA-graph replay: this step's counters live on the device
+        n_pt = dc->n_pt;
+        series_row = dc->series_base ? dc->series_base + (size_t)dc->row * R * 5 : nullptr;
+    }
     for (int k = threadIdx.x >> 5; k < R; k += 32)
         finalize_rank(partials, n_tiles, k, slot_at_rank[k], threadIdx.x & 31, obs_rank, obs_slot, series_row);
     __syncthreads();
@@ -187,6 +201,10 @@ __global__ void __launch_bounds__(1024) finalize_pt_kernel(const double* __restr
             beta32_of_slot[a] = (float)betas[k + 1]; beta32_of_slot[b] = (float)betas[k];
             pt_acc[k] += 1ull;
         }
+    }
+    if (dc) {
+        __syncthreads();
+        if (threadIdx.x == 0) { dc->n_met += 1u; dc->n_or += (uint32_t)or_per_mcs; dc->n_pt += 1u; dc->row += 1u; }
     }
 }
 

@@ -43,7 +43,8 @@ struct SweepParams {
     int nItems;                  // TY * W4 own float4 per plane (<= blockDim.x)
     unsigned int half_n;         // L^3 / 2 floats per slot per colour
     PhiloxKeys keys;
-    uint32_t sweep;              // n_met (Philox counter word 2)
+    uint32_t sweep;              // n_met (Philox counter word 2) ...
+    const uint32_t* d_counters;  // ... or, when not null, read from d_counters[0] (CUDA-graph replay: see DeviceCounters)
     const float* beta32_of_slot; // Metropolis: fp32 beta label per slot (R13)
     unsigned long long* met_acc; // Metropolis: accepted proposals per slot
     unsigned long long* exact_count;  // Metropolis: decisions re-evaluated in fp64
@@ -302,7 +303,7 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 384, XY_SWEEP_MIN_BLOCK
             beta32 = P.beta32_of_slot[slot];
             bl = beta32 * 1.44269504f;               // exp(beta g) = 2^(bl g)
             win24 = (fabsf(beta32) * kWindowPerBeta + kWindowAbs) * 4294967296.0f;  // window in units of 2^-32, see xy_device.cuh
-            inv = philox_block_invariants((uint32_t)slot, P.sweep, P.colour == 0 ? kStreamMetBlack : kStreamMetWhite, P.keys);
+            inv = philox_block_invariants((uint32_t)slot, P.d_counters ? P.d_counters[0] : P.sweep, P.colour == 0 ? kStreamMetBlack : kStreamMetWhite, P.keys);
             keep(bl); keep(win24); keep(inv.j0); keep(inv.j1); keep(inv.j2); keep(inv.j3);
         }
         // (cos, sin) pairs of the other colour at this thread's own (y, x) position on three consecutive

@@ -578,6 +578,37 @@ def test_mcs_with_several_overrelaxation_sweeps(xy_mod):
     assert np.array_equal(series.cpu().numpy(), np.stack(rows))
 
 
+@pytest.mark.parametrize("L,R,fused,n_or", [(8, 8, 1, 1), (32, 5, 1, 2), (32, 3, 0, 1), (64, 2, 1, 1)])
+def test_mcs_graph_replay_equals_eager_launches(xy_mod, L, R, fused, n_or):
+    """XY_OPT_CUDA_GRAPH: xy_mcs replays one captured graph per step with the counters on the device.
+    States, permutations, counters, acceptance counts and the observable series must equal, bit for
+    bit, those of eagerly launched steps -- over two calls, so the graph is re-used with new counters."""
+    import torch
+    betas = inputs.beta_ladder(0.45, 0.46, R)
+    runs = []
+    for graph in (1, 0):
+        xy = xy_mod.XY(L, R, betas, SEED)
+        xy.set_option(xy_mod.XY_OPT_CUDA_GRAPH, graph)
+        xy.set_option(xy_mod.XY_OPT_FUSED_MEASURE, fused)
+        xy.set_option(xy_mod.XY_OPT_OR_PER_MCS, n_or)
+        xy.init_random()
+        s1 = torch.zeros(7, R, 5, dtype=torch.float64, device="cuda")
+        s2 = torch.zeros(5, R, 5, dtype=torch.float64, device="cuda")
+        n0 = xy.get_launch_count()
+        xy.mcs(7, s1)
+        xy.mcs(5, s2)
+        xy.mcs(4)                                             # no series
+        runs.append((xy.get_state(), xy.get_perm(), xy.get_counters(), xy.get_accept_counts(), s1.cpu().numpy(),
+                     s2.cpu().numpy(), xy.measure(), xy.get_launch_count() - n0))
+    a, b = runs
+    assert np.array_equal(a[0].view(np.uint32), b[0].view(np.uint32))
+    assert np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2]) and np.array_equal(a[2], [16, 16 * n_or, 16])
+    assert np.array_equal(a[3][0], b[3][0]) and np.array_equal(a[3][1], b[3][1])
+    assert np.array_equal(a[4], b[4]) and np.array_equal(a[5], b[5]) and np.array_equal(a[6], b[6])
+    assert np.all(a[4][:, :, 3] > 0)                          # every row was written
+    assert a[7] == b[7] + 3, "same kernels per step, plus one counter upload per call"
+
+
 # ---- P7: long-run statistics ---------------------------------------------------------------------
 def _run_means(series, N):
     """series [T,R,5] (after the discarded head) -> time averages E/N [R] and Q2 = <M4>/<M2>^2 [R]."""
