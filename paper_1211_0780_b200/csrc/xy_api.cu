@@ -134,14 +134,14 @@ void default_tiles(int L, int R, int& TY, int& TZ) {
     for (int t = 8; t <= L; ++t)
         if (L % t == 0 && t * W4 <= 320) TY = t;
     // March length: a block costs TZ + 2 steps (two of them only stage) and 2 blocks fit an SM, so
-    // the pass takes about ceil(blocks / (2 * 148 SMs)) * (TZ + 1/2) step-times: take the divisor of L
+    // the pass takes about ceil(blocks / (2 * 148 SMs)) * (TZ + 1) step-times: take the divisor of L
     // that minimises it (the last, partly filled wave is what a long march wastes).
     TZ = L;
     double best = 1e300;
-    for (int t = L; t >= 8; --t) {
+    for (int t = L; t >= 2; --t) {
         if (L % t) continue;
         const long blocks = (long)R * (L / TY) * (L / t);
-        const double cost = (double)((blocks + 295) / 296) * (t + 0.5);
+        const double cost = (double)((blocks + 295) / 296) * (t + 1.0);
         if (cost < best * 0.999) { best = cost; TZ = t; }
     }
 }
