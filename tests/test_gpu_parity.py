@@ -609,6 +609,32 @@ def test_mcs_graph_replay_equals_eager_launches(xy_mod, L, R, fused, n_or):
     assert a[7] == b[7] + 3, "same kernels per step, plus one counter upload per call"
 
 
+def test_user_stream_and_context_lifetime(xy_mod):
+    """A caller-owned (non-blocking) torch stream: same results as the library's own stream, graph replay
+    included; and contexts can be created and destroyed repeatedly without leaking device memory."""
+    import torch
+    L, R = 32, 4
+    betas = inputs.beta_ladder(0.45, 0.46, R)
+    ref = xy_mod.XY(L, R, betas, SEED)
+    ref.init_random(); ref.mcs(6)
+    want = ref.get_state()
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        xy = xy_mod.XY(L, R, betas, SEED, stream=st)
+        xy.init_random(); xy.mcs(6)
+        got = xy.get_state()
+    assert np.array_equal(got.view(np.uint32), want.view(np.uint32))
+    xy.close(); ref.close()
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    for _ in range(40):
+        t = xy_mod.XY(L, R, betas, SEED)
+        t.init_random(); t.mcs(3); t.measure()
+        t.close()
+    torch.cuda.synchronize()
+    assert free0 - torch.cuda.mem_get_info()[0] < 64 << 20
+
+
 # ---- P7: long-run statistics ---------------------------------------------------------------------
 def _run_means(series, N):
     """series [T,R,5] (after the discarded head) -> time averages E/N [R] and Q2 = <M4>/<M2>^2 [R]."""
