@@ -457,6 +457,27 @@ def test_full_mcs_lockstep_on_configs(xy_mod, oracle_mod, idx, n_mcs):
         t += 1
 
 
+@pytest.mark.parametrize("L,R", [(80, 3), (96, 2)])
+def test_paper_other_sizes_and_nonuniform_ladder(xy_mod, oracle_mod, L, R):
+    """the paper's L = 80 and 96 have no compile-time kernel variant (their rows do
+    not split into whole warps per parity class) and its temperature ladders are not uniform: the
+    run-time-geometry kernel on a non-uniformly spaced, unsorted beta set, lock-step against the oracle."""
+    betas = np.array([1.0 / 2.2019, 1.0 / 2.25, 1.0 / 2.19][:R])          # T_c of P:76 and two neighbours, unsorted
+    xy, ora = make(xy_mod, oracle_mod, L, R, betas=betas)
+    xy.init_random()
+    t = 0
+    for s in (0, 1, 5):
+        if s > t:
+            xy.mcs(s - t)
+            t = s
+        mcs_lockstep(xy, ora, t)
+        t += 1
+    g, o = xy.measure_stiffness(), None
+    ora.set_state(xy.get_state()); ora.set_perm(xy.get_perm())
+    o = ora.measure_stiffness()
+    assert np.all(np.abs(g - o) <= 4e-6 * L ** 3)
+
+
 def test_free_run_divergence_report(xy_mod, oracle_mod):
     """P6: GPU and oracle run freely from the same start.  Only k = 1 is asserted (chaos: the
     difference grows x3-5 per MCS, SURVEY.md finding 3); the curve is printed."""
