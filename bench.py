@@ -164,6 +164,8 @@ def run_ours(args, cfg):
         xy.init_random()
     else:
         xy.init_ordered(0.0)
+    if args.tile_y:
+        xy.set_option(binding.XY_OPT_TILE_Y, args.tile_y)
     if args.tile_z:
         xy.set_option(binding.XY_OPT_TILE_Z, args.tile_z)
     if args.generic_kernel:
@@ -279,6 +281,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--tile-z", type=int, default=0, help="override the march length (tuning; 0 = library default)")
+    ap.add_argument("--tile-y", type=int, default=0, help="override the tile rows (tuning; 0 = library default)")
     ap.add_argument("--generic-kernel", action="store_true", help="force the run-time-geometry colour-pass kernel (tuning)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
