@@ -62,16 +62,6 @@ __device__ __forceinline__ f32x2 pack2(float lo, float hi) { f32x2 d; asm("mov.b
 __device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
 __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
-// y + (par ? x1 : x0) as two predicated packed additions (one executes): no 64-bit selects
-__device__ __forceinline__ f32x2 add2_sel(f32x2 y, f32x2 x0, f32x2 x1, int par) {
-    f32x2 d;
-    asm("{\n .reg .pred p;\n setp.ne.s32 p, %4, 0;\n @p add.rn.f32x2 %0, %1, %3;\n @!p add.rn.f32x2 %0, %1, %2;\n}"
-        : "=l"(d) : "l"(y), "l"(x0), "l"(x1), "r"(par));
-    return d;
-}
-
-__device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
-
 // ---- mbarrier (shared::cta): the split arrive / wait block barrier -------------------------------
 __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
