@@ -294,6 +294,17 @@ def test_exact_L2_quadrature_converged():
     assert abs(e10 - (-12.961145712)) < 2e-6                   # SURVEY.md O9 (3-D Bessel quadrature) cross-check
 
 
+def test_exact_L2_quadrature_matches_the_stored_values():
+    """tests/golden/l2_exact_energy.txt (an independent Bessel-function quadrature) against this
+    repository's own brute-force 7-D grid: two routes to the same numbers, four temperatures."""
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "l2_exact_energy.txt"))
+            if l.strip() and not l.startswith("#")]
+    assert len(rows) == 4
+    for beta, want in rows:
+        M = 14 if float(beta) >= 1.0 else 10                  # the integrand sharpens with beta
+        assert abs(H.exact_mean_energy_L2(float(beta), M) - float(want)) < 5e-6, beta
+
+
 @pytest.mark.parametrize("with_or", [False, True])
 def test_O9_L2_mean_energy_against_brute_force(oracle_mod, with_or):
     beta, R, T, burn = 0.45, 64, 6000, 50
