@@ -305,10 +305,10 @@ def test_exact_L2_quadrature_matches_the_stored_values():
         assert abs(H.exact_mean_energy_L2(float(beta), M) - float(want)) < 5e-6, beta
 
 
-@pytest.mark.parametrize("with_or", [False, True])
-def test_O9_L2_mean_energy_against_brute_force(oracle_mod, with_or):
-    beta, R, T, burn = 0.45, 64, 6000, 50
-    want = H.exact_mean_energy_L2(beta, 10)
+@pytest.mark.parametrize("beta,with_or", [(0.45, False), (0.45, True), (0.2, True), (1.0, True), (1.0, False)])
+def test_O9_L2_mean_energy_against_brute_force(oracle_mod, beta, with_or):
+    R, T, burn = 64, 6000, 50
+    want = H.exact_mean_energy_L2(beta, 14 if beta >= 1.0 else 10)
     o = oracle_mod.XYOracle(2, R, np.full(R, beta), SEED + (1 if with_or else 0))
     o.init_random()
     E = np.empty((T, R))
