@@ -656,6 +656,37 @@ def test_user_stream_and_context_lifetime(xy_mod):
     assert free0 - torch.cuda.mem_get_info()[0] < 64 << 20
 
 
+def test_gpu_sampler_against_closed_forms(xy_mod):
+    """The GPU chain pinned to mathematics instead of to the oracle:
+    high-temperature series <cos> per bond = t + 8 t^3 t' (t = I1/I0) at beta = 0.1, with the exchanges on
+    (all beta equal: every attempted pair swaps, which must not change anything); beta = 0 gives <E> = 0;
+    and the ordered state at huge beta is a fixed point of the whole step with E/N = -3."""
+    import torch
+    from scipy.special import i0, i1
+    L, R, T, burn = 16, 32, 400, 20
+    N = L ** 3
+    for beta in (0.1, 0.0):
+        xy = xy_mod.XY(L, R, np.full(R, beta), SEED + 7)
+        xy.init_random()
+        series = torch.zeros(burn + T, R, 5, dtype=torch.float64, device="cuda")
+        xy.mcs(burn + T, series)
+        e = series.cpu().numpy()[burn:, :, 0] / N
+        mean, err = H.mean_and_err_over_replicas(e)
+        if beta > 0:
+            t = i1(beta) / i0(beta)
+            want = -3 * (t + 8 * t ** 3 * (1 - t / beta - t * t))
+        else:
+            want = 0.0
+        print("beta", beta, "E/N", mean, "+-", err, "want", want)
+        assert err < 3e-4 and abs(mean - want) < 4 * err + 2e-4, (beta, mean, want, err)
+    xy = xy_mod.XY(L, 4, np.full(4, 1e30), SEED)
+    xy.init_ordered(0.0)
+    xy.mcs(5)
+    assert np.array_equal(xy.get_state(), np.zeros((4, L, L, L), dtype=np.float32))
+    o = xy.measure()
+    assert np.allclose(o[:, 0], -3.0 * N) and np.allclose(o[:, 1], N) and np.allclose(o[:, 2], 0.0)
+
+
 # ---- P7: long-run statistics ---------------------------------------------------------------------
 def _run_means(series, N):
     """series [T,R,5] (after the discarded head) -> time averages E/N [R] and Q2 = <M4>/<M2>^2 [R]."""
