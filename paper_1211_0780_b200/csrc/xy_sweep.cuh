@@ -139,7 +139,7 @@ __host__ __device__ inline size_t sweep_smem_bytes(int L, int TY) {
 #define XY_SWEEP_MIN_BLOCKS 2
 #endif
 template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE, int W4C, int TYC>
-__global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 384, XY_SWEEP_MIN_BLOCKS) sweep_kernel(const SweepParams P) {
+__global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 384, (W4C * TYC > 352) ? 1 : XY_SWEEP_MIN_BLOCKS) sweep_kernel(const SweepParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr bool UNI = W4C != 0;
     const int L = P.L;
