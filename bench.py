@@ -99,8 +99,18 @@ def combine_ranks(ms_local, units_local, dist=None, device="cpu"):
     return float(t.item()), float(u.item())
 
 
+NCU_PEAK_GBS = 8184.0          # ncu's own denominator for dram % of peak: 3996 MHz x 8192 bit x 2
+
+
+def config_keys(cfg):
+    """The workload description both arms print (the reference arm adds what it sampled)."""
+    return {"workload": cfg.name, "L": cfg.L, "R": cfg.R, "beta": [cfg.beta_lo, cfg.beta_hi], "start": cfg.start,
+            "state_bytes": 4 * cfg.L ** 3 * cfg.R}
+
+
 def oracle_sample_rate(cfg, n_slots, steps, warmup, threads):
-    """The CPU oracle, as it stands, on a bounded sample: full MCS of the first n_slots temperatures of cfg."""
+    """The CPU oracle, as it stands, on a bounded sample: full MCS of the first n_slots temperatures of cfg.
+    XYOracle.mcs() reduces the observables once per step and hands the energies to the exchange."""
     from oracle import xy_oracle
     betas = inputs.betas_of(cfg)[:n_slots]
     ora = xy_oracle.XYOracle(cfg.L, n_slots, betas, inputs.SEED, threads=threads)
@@ -130,8 +140,9 @@ def run_reference(args, cfg):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg.name, "L": cfg.L, "R": cfg.R, "sampled_replicas": n_slots},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": n_slots, "kind": "oracle", "sample": sample},
+        "config": dict(config_keys(cfg), sampled_replicas=n_slots),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": n_slots, "kind": "oracle", "sample": sample,
+                         "ns_per_update_per_core": n_slots / value},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
@@ -243,15 +254,19 @@ def run_ours(args, cfg):
         "metric": METRIC, "value": units / (ms * 1e-3) * 1e-9, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": cfg.name, "L": L, "R": R, "beta": [cfg.beta_lo, cfg.beta_hi], "start": cfg.start,
-                   "state_bytes": 4 * N * R, "l2": "inputs larger than L2 (state 1.05 GB >> 126 MB)" if 4 * N * R > 4e8
-                   else "state fits in L2; no flush", "parallelism": "replicas only" if world > 1 else "1 GPU",
-                   "tile_y": xy.get_option(binding.XY_OPT_TILE_Y), "tile_z": xy.get_option(binding.XY_OPT_TILE_Z)},
+        "config": dict(config_keys(cfg), l2=f"inputs larger than L2 (state {4 * N * R / 1e9:.2f} GB >> 126 MB)" if 4 * N * R > 4e8
+                   else "state fits in L2; no flush", parallelism="replicas only" if world > 1 else "1 GPU",
+                   tile_y=xy.get_option(binding.XY_OPT_TILE_Y), tile_z=xy.get_option(binding.XY_OPT_TILE_Z)),
         "site_mcs_per_ns": units / 2 / (ms * 1e-3) * 1e-9,
         "hbm_roofline_frac_whole_mcs": units * BYTES_PER_UPDATE / (ms * 1e-3) * 1e-9 / peak,
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
                      "frac": ach / peak, "traffic": traffic, "bytes_per_update": BYTES_PER_UPDATE,
-                     "algorithmic_bytes_per_launch": per_launch_bytes[dom]},
+                     "algorithmic_bytes_per_launch": per_launch_bytes[dom],
+                     # the second denominator SURVEY.md 8(d) asks for, labelled: ncu's theoretical DRAM peak, and the
+                     # dram throughput % ncu itself reported for this kernel in the committed capture (profiles/)
+                     "frac_of_ncu_peak": ach / NCU_PEAK_GBS, "ncu_peak": NCU_PEAK_GBS,
+                     "ncu_dram_pct_of_peak_sustained_elapsed": NCU_TRAFFIC_BYTES.get(cfg.name, {}).get(dom + "_dram_pct")},
+        "hbm_roofline_frac_whole_mcs_of_ncu_peak": units * BYTES_PER_UPDATE / (ms * 1e-3) * 1e-9 / NCU_PEAK_GBS,
         "kernels": kern,
         "kernels_measured": f"second pass of {args.steps} steps with a CUDA-event pair around every launch: {ms_profiled / args.steps:.4f} ms per step",
         "e2e": {"value": e2e_units / (e2e_ms * 1e-3) * 1e-9, "unit": UNIT, "h2d_bytes_per_step": 4 * N * R,
@@ -267,7 +282,8 @@ def run_ours(args, cfg):
         v, _ = oracle_sample_rate(cfg, n_slots, 2, 1, threads=n_slots)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": n_slots, "kind": "oracle",
                                "sample": f"2 timed MCS (after 1 warm-up) of the first {n_slots} of {R} temperatures at L={L}, "
-                                         "one thread per replica"}
+                                         "one thread per replica; one reduction per step",
+                               "ns_per_update_per_core": n_slots / v, "gpu_over_cpu": out["value"] / v}
     print(json.dumps(out))
 
 

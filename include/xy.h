@@ -97,8 +97,10 @@ size_t xy_state_bytes(int L, int R);
 size_t xy_workspace_bytes(int L, int R);
 
 /* Binds device memory and a stream.  d_state / d_workspace: DEVICE pointers, 256-byte aligned,
- * of at least xy_state_bytes / xy_workspace_bytes, owned by the caller (PyTorch) and required to
- * outlive the context; either may be NULL, in which case the library cudaMallocs and owns it.
+ * of at least xy_state_bytes / xy_workspace_bytes, on the CURRENT device, owned by the caller
+ * (PyTorch) and required to outlive the context.  The context is bound to the device that is
+ * current at this call: every later entry point switches to it for its own duration and restores
+ * the caller's current device.  Either buffer may be NULL, in which case the library cudaMallocs and owns it.
  * cuda_stream: a cudaStream_t; NULL = the library creates a blocking stream of its own, which is
  * implicitly ordered with the legacy default stream (that one cannot be captured into a CUDA graph).  Uploads the beta labels and
  * the identity permutation; the spin state is undefined until xy_init_* or xy_set_state. */
@@ -117,7 +119,9 @@ int xy_init_ordered(xy_ctx* ctx, float theta0);
  * host pointer (pinned memory makes the copy asynchronous-capable; the call synchronises
  * before returning for xy_get_state, and before the host buffer may be reused for
  * xy_set_state); on_device = 1: a device pointer readable from the attached stream, no
- * synchronisation.  The layout conversion runs in a kernel. */
+ * synchronisation.  The layout conversion runs in a kernel.  The kernels' stated errors hold for
+ * angles in [0, 2 pi]: xy_set_state reduces any finite angle outside that range modulo 2 pi
+ * (angles inside it are stored bit for bit); a NaN or infinite angle is stored as 0. */
 int xy_set_state(xy_ctx* ctx, const float* natural, int on_device);
 int xy_get_state(xy_ctx* ctx, float* natural, int on_device);
 
@@ -128,9 +132,14 @@ int xy_get_state(xy_ctx* ctx, float* natural, int on_device);
  * of (cos, sin) [P:23-28 Eq. 1]:  W = Philox(counter = (i>>2, r, n_met, 1 + colour)),
  * p = (i>>1)&1, theta' = fl32(2pi_f * u24(W[2p])), dE = -h.(S(theta') - S(theta)),
  * accept iff u24(W[2p+1]) < exp(-fl32(beta_of_slot[r]) * dE)  [R1, R2, R12, R13].
- * The decision is taken in fp32 fast arithmetic when it is clear and re-evaluated in fp64
- * from the stored angles when |u - p_fast| < 2^-14, so it equals the fp64 definition
- * (DESIGN.md section 6).  Accepted angles are bit-identical to the definition.  ++n_met. */
+ * The decision is taken in fp32 fast arithmetic when it is clear.  When |u - p_fast| is inside the
+ * window |beta| * 4e-5 + 1.5e-6 (the derived bound of the fast path's error, csrc/xy_device.cuh) the
+ * site is appended to a device queue and settled by met_fixup_kernel in fp64 from the stored
+ * angles right after the colour pass (for very large |beta|, where most decisions are close, in
+ * the pass itself), so every decision equals the fp64 definition.  Accepted
+ * angles are bit-identical to the definition.  Should a pass ever produce more close decisions
+ * than the queue holds, a sticky flag makes every later synchronising call return XY_ERR_CUDA
+ * ("queue overflowed") until the context is attached again: results are then not exact.  ++n_met. */
 int xy_metropolis_sweep(xy_ctx* ctx);
 
 /* One checkerboard over-relaxation sweep, black then white: theta' = 2*atan2(h_y, h_x) - theta

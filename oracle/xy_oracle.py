@@ -218,9 +218,13 @@ class XYOracle:
             _chk(lib().xyo_pt_exchange_with_E(self._h, _p(e, C.c_double)), "pt_exchange_with_E")
 
     def mcs(self):
-        """one Metropolis sweep, one over-relaxation sweep, then one PT exchange."""
+        """one Metropolis sweep, one over-relaxation sweep, then one PT exchange.  The observables are
+        reduced ONCE per step: the by-slot energies that xyo_measure_slots returns are handed to
+        xyo_pt_exchange_with_E (xyo_pt_exchange would reduce every slot a second time).  Returns them by rank,
+        as they were before the exchange (R14)."""
         self.metropolis_sweep()
         self.overrelax_sweep()
-        obs = self.measure()
-        self.pt_exchange()
+        by_slot = self.measure_slots()
+        obs = by_slot[self.get_perm()]
+        self.pt_exchange(by_slot[:, 0])
         return obs

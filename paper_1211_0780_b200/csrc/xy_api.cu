@@ -2,6 +2,7 @@
 // Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -shared -Xcompiler -fPIC
 #include "../../include/xy.h"
 
+#include <atomic>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -30,6 +31,7 @@ int fail(int code, const char* fmt, ...) {
         if (e_ != cudaSuccess) return fail(XY_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); \
     } while (0)
 
+constexpr int kMaxDevices = 64;
 size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 bool shape_ok(int L, int R) { return L >= 8 && L % 8 == 0 && L <= 1024 && R >= 1 && R <= 65535; }
 size_t max_tiles(int L) { return (size_t)(L / 2) * (size_t)(L / 2); }   // tiles_ok: TY >= 2 and TZ >= 2
@@ -77,6 +79,7 @@ struct xy_ctx {
     PhiloxKeys keys;
     uint32_t n_met = 0, n_or = 0, n_pt = 0;
     // device
+    int device = -1;                           // the CUDA device of the attached buffers and stream (xy_attach)
     bool attached = false;
     float* d_state = nullptr; bool own_state = false;
     char* d_ws = nullptr; bool own_ws = false;
@@ -130,8 +133,8 @@ struct LaunchSpan {
 
 void default_tiles(int L, int R, int& TY, int& TZ) {
     const int W4 = L / 8;
-    TY = 8;
-    for (int t = 8; t <= L; ++t)
+    TY = 2;                                        // L up to 1024: TY * L/8 must stay within 11 compute warps
+    for (int t = 2; t <= L; ++t)
         if (L % t == 0 && t * W4 <= 320) TY = t;
     // March length: a block costs TZ + 2 steps (two of them only stage) and 2 blocks fit an SM, so
     // the pass takes about ceil(blocks / (2 * 148 SMs)) * (TZ + 1) step-times: take the divisor of L
@@ -153,10 +156,12 @@ bool tiles_ok(int L, int TY, int TZ) {
 
 template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE, int W4C, int TYC>
 int launch_sweep_impl(xy_ctx* c, const SweepParams& P) {
-    static bool attr_set = false;
-    if (!attr_set) {
+    // The dynamic-shared-memory opt-in is a per-device attribute of each instantiation: one flag per device,
+    // set outside any stream capture (xy_mcs launches its first step eagerly).
+    static std::atomic<bool> attr_set[kMaxDevices];
+    if (!attr_set[c->device].load(std::memory_order_acquire)) {
         CK(cudaFuncSetAttribute(sweep_kernel<MODE, TRACE, FUSED, EXACT_INLINE, W4C, TYC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_set = true;
+        attr_set[c->device].store(true, std::memory_order_release);
     }
     const size_t smem = sweep_smem_bytes(P.L, P.TY);
     const int threads = (P.nItems + 31) / 32 * 32 + 32;          // compute warps + the auxiliary warp
@@ -216,11 +221,30 @@ SweepParams base_params(xy_ctx* c, int colour) {
     return P;
 }
 
+// Makes the context's device current for the duration of one entry point and restores the caller's.
+struct DeviceScope {
+    int prev = -1; bool switched = false;
+    int enter(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) return fail(XY_ERR_CUDA, "cudaGetDevice failed");
+        if (prev != dev) {
+            if (cudaSetDevice(dev) != cudaSuccess) return fail(XY_ERR_CUDA, "cudaSetDevice(%d) failed", dev);
+            switched = true;
+        }
+        return XY_OK;
+    }
+    ~DeviceScope() { if (switched) cudaSetDevice(prev); }
+};
+
 int need(xy_ctx* c) {
     if (!c) return fail(XY_ERR_INVALID_ARG, "NULL context");
     if (!c->attached) return fail(XY_ERR_NOT_ATTACHED, "context has no device buffers: call xy_attach first");
     return XY_OK;
 }
+// First statement of every entry point that touches the device: validates the context and switches to its device.
+#define ENTER(c)                                   \
+    if (int rc_ = need(c)) return rc_;             \
+    DeviceScope scope_;                            \
+    if (int rc_ = scope_.enter((c)->device)) return rc_
 
 int upload_labels(xy_ctx* c, const int* perm) {
     const int R = c->R;
@@ -293,6 +317,11 @@ xy_ctx* xy_create(int L, int R, const double* betas, uint64_t seed) {
     c->keys = philox_round_keys((uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32));
     c->ws = ws_layout(L, R);
     default_tiles(L, R, c->TY, c->TZ);
+    if (!tiles_ok(L, c->TY, c->TZ)) {
+        fail(XY_ERR_INVALID_ARG, "xy_create: no valid tile for L=%d (TY=%d TZ=%d)", L, c->TY, c->TZ);
+        delete c;
+        return nullptr;
+    }
     // Measured at L=160: the Metropolis pass is 3 % faster as ONE block of 20 + 1 warps per
     // SM (five compute warps on every scheduler) than as two of 10 + 1; the over-relaxation pass is not.
     if (L == 160 && c->TY == 16) { c->TY_met = 32; c->TZ_met = 32; }
@@ -326,8 +355,18 @@ int xy_attach(xy_ctx* c, void* d_state, void* d_workspace, void* cuda_stream) {
     CK(cudaGetDevice(&dev));
     cudaDeviceProp prop;
     CK(cudaGetDeviceProperties(&prop, dev));
+    if (dev < 0 || dev >= kMaxDevices) return fail(XY_ERR_NO_DEVICE, "xy_attach: device index %d out of range", dev);
+    c->device = dev;
     if (prop.major < 10) return fail(XY_ERR_NO_DEVICE, "xy_attach: device %s is sm_%d%d; built for sm_100a only", prop.name, prop.major, prop.minor);
     if (((uintptr_t)d_state | (uintptr_t)d_workspace) & 255u) return fail(XY_ERR_INVALID_ARG, "xy_attach: buffers must be 256-byte aligned");
+    for (void* p : { d_state, d_workspace }) {        // caller-owned buffers must live on the device this context is bound to
+        if (!p) continue;
+        cudaPointerAttributes pa;
+        if (cudaPointerGetAttributes(&pa, p) != cudaSuccess) { cudaGetLastError(); return fail(XY_ERR_INVALID_ARG, "xy_attach: not a CUDA pointer"); }
+        if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) return fail(XY_ERR_INVALID_ARG, "xy_attach: buffers must be device memory");
+        if (pa.type == cudaMemoryTypeDevice && pa.device != dev)
+            return fail(XY_ERR_INVALID_ARG, "xy_attach: buffer lives on device %d but the current device is %d", pa.device, dev);
+    }
     c->stream = (cudaStream_t)cuda_stream;
     if (!c->stream) {                          // the legacy default stream cannot be captured into a graph: use a
         CK(cudaStreamCreate(&c->stream));      // BLOCKING stream of our own, which stays ordered with it
@@ -345,7 +384,7 @@ int xy_attach(xy_ctx* c, void* d_state, void* d_workspace, void* cuda_stream) {
 }
 
 int xy_init_random(xy_ctx* c) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     const size_t n_quads = (size_t)c->R * c->L * c->L * (c->L / 4);
     {
         LaunchSpan span(c, XY_K_OTHER);
@@ -357,7 +396,7 @@ int xy_init_random(xy_ctx* c) {
 }
 
 int xy_init_ordered(xy_ctx* c, float theta0) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     const size_t n = (size_t)c->R * c->N;
     {
         LaunchSpan span(c, XY_K_OTHER);
@@ -397,20 +436,20 @@ static int convert_state(xy_ctx* c, float* black, float* white, float* natural, 
 }
 
 int xy_set_state(xy_ctx* c, const float* natural, int on_device) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     if (!natural) return fail(XY_ERR_INVALID_ARG, "xy_set_state: NULL pointer");
     c->partials_valid = false;
     return convert_state(c, c->colour(0), c->colour(1), const_cast<float*>(natural), on_device, true);
 }
 
 int xy_get_state(xy_ctx* c, float* natural, int on_device) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     if (!natural) return fail(XY_ERR_INVALID_ARG, "xy_get_state: NULL pointer");
     return convert_state(c, c->colour(0), c->colour(1), natural, on_device, false);
 }
 
 int xy_metropolis_sweep(xy_ctx* c) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     if (c->trace && !c->d_trace) CK(cudaMalloc(&c->d_trace, (size_t)c->R * c->N * 4));
     for (int colour = 0; colour < 2; ++colour) {
         SweepParams P = base_params(c, colour);
@@ -457,12 +496,12 @@ static int overrelax_sweep_impl(xy_ctx* c, bool with_observables) {
 }
 
 int xy_overrelax_sweep(xy_ctx* c) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     return overrelax_sweep_impl(c, c->fused != 0);
 }
 
 int xy_measure(xy_ctx* c, double* out) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     if (int rc = run_measure(c, nullptr)) return rc;
     if (out) {
         CK(cudaMemcpyAsync(out, c->ws_ptr<double>(c->ws.obs_rank), (size_t)c->R * 5 * 8, cudaMemcpyDeviceToHost, c->stream));
@@ -505,7 +544,7 @@ static int pt_exchange_impl(xy_ctx* c, double* d_series_row) {
 }
 
 int xy_measure_stiffness(xy_ctx* c, double* out) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     if (!out) return fail(XY_ERR_INVALID_ARG, "xy_measure_stiffness: NULL pointer");
     SweepParams P = base_params(c, 1);         // own = white, staged = black
     P.partials = c->ws_ptr<double>(c->ws.partials6);
@@ -523,7 +562,7 @@ int xy_measure_stiffness(xy_ctx* c, double* out) {
 }
 
 int xy_pt_exchange(xy_ctx* c) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     return pt_exchange_impl(c, nullptr);
 }
 
@@ -560,7 +599,7 @@ static int build_step_graph(xy_ctx* c, uint64_t key) {
 }
 
 int xy_mcs(xy_ctx* c, int n_mcs, double* d_series) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     if (n_mcs < 0) return fail(XY_ERR_INVALID_ARG, "xy_mcs: n_mcs < 0");
     int t = 0;
     // XY_OPT_CUDA_GRAPH: from the second step on, replay one captured graph per step (7 kernel nodes):
@@ -577,11 +616,16 @@ int xy_mcs(xy_ctx* c, int n_mcs, double* d_series) {
         v.n_met = c->n_met; v.n_or = c->n_or; v.n_pt = c->n_pt; v.row = 1u; v.series_base = d_series;
         set_device_counters_kernel<<<1, 1, 0, c->stream>>>(c->ws_ptr<DeviceCounters>(c->ws.dctr), v);
         CK(cudaGetLastError());
-        for (; t < n_mcs; ++t) CK(cudaGraphLaunch(c->graph_exec, c->stream));
-        c->n_met += (uint32_t)(n_mcs - 1); c->n_or += (uint32_t)(n_mcs - 1) * (uint32_t)c->or_per_mcs; c->n_pt += (uint32_t)(n_mcs - 1);
-        c->launches += c->graph_launches * (uint64_t)(n_mcs - 1) + 1;
-        c->partials_valid = true;                  // the step's exchange reduced the final state (labels move, spins do not)
-        c->rank_valid = false;
+        ++c->launches;                             // the counter upload
+        for (; t < n_mcs; ++t) {
+            // the host counters follow every replay that was enqueued, so that a failing launch leaves them equal
+            // to the device's (DeviceCounters) instead of n_mcs - t steps behind
+            CK(cudaGraphLaunch(c->graph_exec, c->stream));
+            c->n_met += 1u; c->n_or += (uint32_t)c->or_per_mcs; c->n_pt += 1u;
+            c->launches += c->graph_launches;
+            c->partials_valid = true;              // the step's exchange reduced the final state (labels move, spins do not)
+            c->rank_valid = false;
+        }
         return XY_OK;
     }
     for (; t < n_mcs; ++t)
@@ -590,7 +634,7 @@ int xy_mcs(xy_ctx* c, int n_mcs, double* d_series) {
 }
 
 int xy_get_perm(xy_ctx* c, int* p) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     if (!p) return fail(XY_ERR_INVALID_ARG, "xy_get_perm: NULL pointer");
     CK(cudaMemcpyAsync(p, c->ws_ptr<int>(c->ws.slot_at_rank), c->R * 4, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
@@ -598,7 +642,7 @@ int xy_get_perm(xy_ctx* c, int* p) {
 }
 
 int xy_set_perm(xy_ctx* c, const int* p) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     if (!p) return fail(XY_ERR_INVALID_ARG, "xy_set_perm: NULL pointer");
     std::vector<char> seen(c->R, 0);
     for (int k = 0; k < c->R; ++k) {
@@ -609,7 +653,7 @@ int xy_set_perm(xy_ctx* c, const int* p) {
 }
 
 int xy_get_beta_of_slot(xy_ctx* c, double* b) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     if (!b) return fail(XY_ERR_INVALID_ARG, "xy_get_beta_of_slot: NULL pointer");
     CK(cudaMemcpyAsync(b, c->ws_ptr<double>(c->ws.beta_of_slot), c->R * 8, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
@@ -629,7 +673,7 @@ int xy_set_counters(xy_ctx* c, const uint32_t n[3]) {
 }
 
 int xy_get_accept_counts(xy_ctx* c, uint64_t* met, uint64_t* pt) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     if (met) CK(cudaMemcpyAsync(met, c->ws_ptr<char>(c->ws.met_acc), c->R * 8, cudaMemcpyDeviceToHost, c->stream));
     if (pt && c->R > 1) CK(cudaMemcpyAsync(pt, c->ws_ptr<char>(c->ws.pt_acc), (c->R - 1) * 8, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
@@ -637,7 +681,7 @@ int xy_get_accept_counts(xy_ctx* c, uint64_t* met, uint64_t* pt) {
 }
 
 int xy_get_exact_path_count(xy_ctx* c, uint64_t* n) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     if (!n) return fail(XY_ERR_INVALID_ARG, "xy_get_exact_path_count: NULL pointer");
     CK(cudaMemcpyAsync(n, c->ws_ptr<char>(c->ws.exact), 8, cudaMemcpyDeviceToHost, c->stream));
     return check_near_overflow(c);
@@ -680,7 +724,7 @@ int xy_get_option(xy_ctx* c, int option, int* value) {
 }
 
 int xy_get_kernel_times(xy_ctx* c, double* ms, uint64_t* n) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     if (!ms || !n) return fail(XY_ERR_INVALID_ARG, "xy_get_kernel_times: NULL pointer");
     CK(cudaStreamSynchronize(c->stream));
     for (auto& s : c->spans) {
@@ -703,12 +747,12 @@ int xy_get_launch_count(xy_ctx* c, uint64_t* n) {
 }
 
 int xy_synchronize(xy_ctx* c) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     return check_near_overflow(c);
 }
 
 int xy_debug_get_trace(xy_ctx* c, float* natural) {
-    if (int rc = need(c)) return rc;
+    ENTER(c);
     if (!natural) return fail(XY_ERR_INVALID_ARG, "xy_debug_get_trace: NULL pointer");
     if (!c->d_trace) return fail(XY_ERR_INVALID_ARG, "xy_debug_get_trace: no trace recorded (set XY_OPT_TRACE before the sweep)");
     return convert_state(c, c->d_trace, c->d_trace + (size_t)c->R * c->half_n, natural, 0, false);

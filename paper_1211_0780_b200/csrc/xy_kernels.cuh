@@ -236,6 +236,19 @@ __global__ void fill_kernel(float* __restrict__ p, size_t n, float v) {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = v;
 }
 
+// The fast sin/cos, the fp64 window and the over-relaxation wrap are all stated for angles in [0, 2 pi]
+// (R7): anything else entering through xy_set_state is reduced modulo 2 pi in double; in-range angles pass
+// bit for bit; NaN / inf become 0.
+__device__ __forceinline__ float angle_in_range(float t) {
+    if (t >= 0.0f && t <= kTwoPiF) return t;
+    if (!(fabsf(t) <= 3.0e38f)) return 0.0f;
+    const double two_pi = 6.283185307179586476925;
+    double r = fmod((double)t, two_pi);
+    if (r < 0.0) r += two_pi;
+    const float f = (float)r;
+    return f > kTwoPiF ? kTwoPiF : f;
+}
+
 // natural [slots][z][y][x] <-> colour-split; one thread per 8 consecutive x (two float4 natural,
 // one float4 per colour).  `slot0` offsets the split arrays (natural points at slot0's first site).
 template <bool TO_SPLIT>
@@ -254,7 +267,9 @@ __global__ void convert_kernel(float* __restrict__ natural, float* __restrict__ 
         float4* ev = reinterpret_cast<float4*>(par == 0 ? black : white) + so;   // even x
         float4* od = reinterpret_cast<float4*>(par == 0 ? white : black) + so;   // odd x
         if (TO_SPLIT) {
-            const float4 a = nat[0], b = nat[1];
+            float4 a = nat[0], b = nat[1];
+            a.x = angle_in_range(a.x); a.y = angle_in_range(a.y); a.z = angle_in_range(a.z); a.w = angle_in_range(a.w);
+            b.x = angle_in_range(b.x); b.y = angle_in_range(b.y); b.z = angle_in_range(b.z); b.w = angle_in_range(b.w);
             *ev = make_float4(a.x, a.z, b.x, b.z);
             *od = make_float4(a.y, a.w, b.y, b.w);
         } else {

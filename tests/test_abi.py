@@ -89,3 +89,57 @@ def test_input_recipe_matches_baseline_json():
         assert b.shape == (c.R,) and b[0] == c.beta_lo and abs(b[-1] - c.beta_hi) < 1e-15
         assert np.all(np.diff(b) > 0)
     assert inputs.HEADLINE.L == 160 and inputs.HEADLINE.R == 64
+
+
+def test_create_accepts_every_documented_lattice_size(xy_mod):
+    """include/xy.h: any L % 8 == 0 up to 1024.  Every such size must get a launchable tile (TY * L/8 within the
+    kernel's launch bounds, shared memory within the opt-in limit): xy_create checks it and reports the tile."""
+    lib = xy_mod.load_library()
+    b = np.array([0.45])
+    pb = b.ctypes.data_as(C.POINTER(C.c_double))
+    for L in range(8, 1025, 8):
+        h = lib.xy_create(L, 1, pb, 1)
+        assert h, (L, lib.xy_last_error())
+        ty, tz = C.c_int(0), C.c_int(0)
+        assert lib.xy_get_option(h, 1, C.byref(ty)) == 0 and lib.xy_get_option(h, 2, C.byref(tz)) == 0
+        assert ty.value >= 2 and L % ty.value == 0 and ty.value * (L // 8) <= 352, (L, ty.value)
+        assert tz.value >= 2 and L % tz.value == 0
+        lib.xy_destroy(h)
+
+
+def test_build_is_stale_after_an_edit_to_any_kernel_header(tmp_path, monkeypatch):
+    """The in-tree .so travels to the GPU box: the builder must never keep a library that was compiled from
+    other sources.  Every file of csrc/ and include/ is a dependency (the colour-pass kernel xy_sweep.cuh was
+    once missing from the list), and touching the CONTENT of any of them makes _stale() true."""
+    import shutil
+    from paper_1211_0780_b200 import build as B
+    names = {os.path.basename(d) for d in B.dependencies()}
+    for f in os.listdir(B.CSRC):
+        if f.endswith((".cu", ".cuh")):
+            assert f in names, f
+    assert {"xy_sweep.cuh", "xy_api.cu", "xy_device.cuh", "xy_kernels.cuh", "xy.h"} <= names
+    csrc, inc = tmp_path / "csrc", tmp_path / "include"
+    shutil.copytree(B.CSRC, csrc)
+    shutil.copytree(B.INCLUDE, inc)
+    lib = tmp_path / "libxy_b200.so"
+    monkeypatch.setattr(B, "CSRC", str(csrc))
+    monkeypatch.setattr(B, "INCLUDE", str(inc))
+    monkeypatch.setattr(B, "LIB_PATH", str(lib))
+    monkeypatch.setattr(B, "HASH_PATH", str(lib) + ".hash")
+    assert B._stale()                                    # no library yet
+    lib.write_bytes(b"")
+    (tmp_path / "libxy_b200.so.hash").write_text(B.source_hash() + "\n")
+    assert not B._stale()
+    for f in ("xy_sweep.cuh", "xy_kernels.cuh", "xy_device.cuh", "xy_api.cu"):
+        with open(csrc / f, "a") as fh:
+            fh.write("// edit\n")
+        assert B._stale(), f
+        (tmp_path / "libxy_b200.so.hash").write_text(B.source_hash() + "\n")
+        assert not B._stale()
+    with open(inc / "xy.h", "a") as fh:
+        fh.write("/* edit */\n")
+    assert B._stale()
+    monkeypatch.setenv("XY_NVCC_EXTRA", "")
+    (tmp_path / "libxy_b200.so.hash").write_text(B.source_hash() + "\n")
+    monkeypatch.setenv("XY_NVCC_EXTRA", "-DXY_SWEEP_MIN_BLOCKS=3")
+    assert B._stale(), "other compiler flags are another library"

@@ -363,6 +363,42 @@ def test_pt_labels_follow_the_permutation_and_eq3_sign(oracle_mod):
     assert list(pt_acc) == [1, 0, 1]
 
 
+def test_pt_uniform_is_predictable_from_philox_alone(oracle_mod):
+    """The exchange DRAW, not only the decision (DESIGN R9 / R12 / R17; Eq. 3): for pair (k, k+1)
+    of exchange number n_pt the uniform is word 0 of Philox(counter = (k, 0, n_pt, stream 3), key = seed),
+    scaled by 2^-32 in double -- predicted here from the independent numpy Philox of tests/helpers.py, for even
+    and odd n_pt (which also fixes which pairs are attempted), several seeds and an R that leaves a last
+    unpaired rank.  A wrong word, counter slot, stream id or scale fails this test."""
+    for seed in (SEED, 0x0123456789ABCDEF, 7):
+        for R in (6, 7):
+            betas = np.linspace(0.40, 0.52, R)
+            o = oracle_mod.XYOracle(4, R, betas, seed)
+            o.init_random()
+            E = np.linspace(-150.0, -90.0, R)                       # by slot; any finite energies will do
+            for n_pt in (0, 1, 2, 5, 4096, 2 ** 32 - 1):
+                o.set_counters([3, 9, n_pt])                        # n_met, n_or must not enter the PT counter
+                perm0 = o.get_perm().copy()
+                tr = o.enable_trace(pt=True)
+                o.pt_exchange(E)
+                ks = np.arange(n_pt & 1, R - 1, 2)
+                w0 = H.philox4x32_10_np(ks, 0, n_pt, H.STREAM_PT, seed & 0xFFFFFFFF, seed >> 32)[0]
+                want_u = w0.astype(np.float64) * 2.0 ** -32
+                got_u = tr["pt_u"]
+                attempted = ~np.isnan(got_u)
+                assert list(np.nonzero(attempted)[0]) == list(ks), (R, n_pt)
+                assert np.array_equal(got_u[ks], want_u), (seed, R, n_pt)
+                assert np.all((want_u >= 0.0) & (want_u < 1.0))
+                # ... and the decision is exactly `u < exp(dbeta dE)` with that u (Eq. 3), pair by pair
+                want_p = np.exp((betas[ks] - betas[ks + 1]) * (E[perm0[ks]] - E[perm0[ks + 1]]))
+                assert np.allclose(tr["pt_p"][ks], want_p, rtol=1e-14)
+                perm = perm0.copy()
+                for k, u, p_ in zip(ks, want_u, want_p):
+                    if u < p_:
+                        perm[k], perm[k + 1] = perm[k + 1], perm[k]
+                assert np.array_equal(o.get_perm(), perm)
+                o.enable_trace()
+
+
 def test_O11_pt_leaves_per_temperature_energy_unchanged(oracle_mod):
     L, R, T, burn = 4, 4, 2500, 100
     betas = np.array([0.40, 0.45, 0.50, 0.55])
