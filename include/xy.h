@@ -61,12 +61,16 @@ enum {
                               time, also for L = 32, 64, 128, 160 where a compile-time variant exists  */
     XY_OPT_OR_PER_MCS = 7, /* over-relaxation sweeps per Monte Carlo step of xy_mcs (default 1, P:30;
                               P:43 "after several sweeps": microcanonical sweeps are cheap decorrelation) */
-    XY_OPT_CUDA_GRAPH = 8  /* 1 (default): xy_mcs replays one captured CUDA graph per step from its second
+    XY_OPT_CUDA_GRAPH = 8, /* 1 (default): xy_mcs replays one captured CUDA graph per step from its second
                               step on (counters live on the device); 0: every kernel is launched eagerly  */
+    XY_OPT_RESIDENT = 9    /* 1 (default): for small lattices (L = 8 ... 48, R <= 512, everything co-resident) xy_mcs
+                              runs all its steps in ONE persistent launch with the spins resident in shared
+                              memory (same results: states, labels and counters bitwise, observables
+                              within the reduction's rounding); 0: always the per-pass kernels                 */
 };
 
 /* Kernel classes reported by xy_get_kernel_times. */
-#define XY_NUM_KERNEL_CLASSES 7
+#define XY_NUM_KERNEL_CLASSES 8
 enum {
     XY_K_METROPOLIS = 0, /* one Metropolis colour pass over all slots (a2)                         */
     XY_K_OVERRELAX = 1,  /* one over-relaxation colour pass over all slots (a3)                    */
@@ -74,7 +78,8 @@ enum {
     XY_K_FINALIZE = 3,   /* a4 final stage: per-slot sums in fixed order, by-rank output           */
     XY_K_PT = 4,         /* the replica-exchange kernel (a5)                                       */
     XY_K_OTHER = 5,      /* init, fill, layout conversion                                          */
-    XY_K_FIXUP = 6       /* a2: fp64 settlement of the close Metropolis decisions of one colour pass */
+    XY_K_FIXUP = 6,      /* a2: fp64 settlement of the close Metropolis decisions of one colour pass */
+    XY_K_RESIDENT = 7    /* a2..a5 of n whole steps in one persistent launch (small lattices, XY_OPT_RESIDENT) */
 };
 
 /* ---- lifetime ------------------------------------------------------------------------------ */
@@ -192,6 +197,11 @@ int xy_get_accept_counts(xy_ctx* ctx, uint64_t* met_acc /* R */, uint64_t* pt_ac
 int xy_get_exact_path_count(xy_ctx* ctx, uint64_t* n);
 int xy_set_option(xy_ctx* ctx, int option, int value);
 int xy_get_option(xy_ctx* ctx, int option, int* value);
+/* How xy_mcs will run on this context (XY_OPT_RESIDENT): out[0] = 1 if all steps of a call run in one persistent
+ * launch with the spins resident in shared memory, else 0 (per-pass kernels); out[1] = slots per thread block,
+ * out[2] = thread blocks (cluster size) per slot, out[3] = threads per block, out[4] = blocks, out[5] = dynamic
+ * shared memory per block in bytes.  The plan needs the device: call after xy_attach. */
+int xy_get_resident_plan(xy_ctx* ctx, int out[6]);
 /* Number of kernels this context has launched since attach (bench.py's gpu_launches). */
 int xy_get_launch_count(xy_ctx* ctx, uint64_t* n);
 /* With XY_OPT_PROFILE = 1: device time in milliseconds (CUDA events on the attached stream) and

@@ -14,8 +14,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libxy_b200.so")
 _lib = None
 
-XY_OPT_TILE_Y, XY_OPT_TILE_Z, XY_OPT_TRACE, XY_OPT_FUSED_MEASURE, XY_OPT_PROFILE, XY_OPT_GENERIC_KERNEL, XY_OPT_OR_PER_MCS, XY_OPT_CUDA_GRAPH = 1, 2, 3, 4, 5, 6, 7, 8
-KERNEL_CLASSES = ("metropolis", "overrelax", "measure", "finalize", "pt", "other", "fixup")
+XY_OPT_TILE_Y, XY_OPT_TILE_Z, XY_OPT_TRACE, XY_OPT_FUSED_MEASURE, XY_OPT_PROFILE, XY_OPT_GENERIC_KERNEL, XY_OPT_OR_PER_MCS, XY_OPT_CUDA_GRAPH, XY_OPT_RESIDENT = 1, 2, 3, 4, 5, 6, 7, 8, 9
+KERNEL_CLASSES = ("metropolis", "overrelax", "measure", "finalize", "pt", "other", "fixup", "resident")
 NUM_OBS = 5
 
 # name -> (restype, argtypes); tests/test_abi.py checks this table against include/xy.h
@@ -48,6 +48,7 @@ SIGNATURES = {
     "xy_set_option": (_i, [_vp, _i, _i]),
     "xy_get_option": (_i, [_vp, _i, _pi]),
     "xy_get_launch_count": (_i, [_vp, _pu64]),
+    "xy_get_resident_plan": (_i, [_vp, _pi]),
     "xy_get_kernel_times": (_i, [_vp, _pd, _pu64]),
     "xy_synchronize": (_i, [_vp]),
     "xy_last_error": (C.c_char_p, []),
@@ -246,6 +247,12 @@ class XY:
         n = C.c_uint64(0)
         _check(_lib.xy_get_launch_count(self._h, C.byref(n)), "xy_get_launch_count")
         return int(n.value)
+
+    def get_resident_plan(self):
+        """{'resident': bool, 'slots_per_block', 'blocks_per_slot', 'threads', 'blocks', 'smem_bytes'} of xy_mcs on this context."""
+        out = (C.c_int * 6)()
+        _check(_lib.xy_get_resident_plan(self._h, out), "xy_get_resident_plan")
+        return dict(zip(("resident", "slots_per_block", "blocks_per_slot", "threads", "blocks", "smem_bytes"), [int(v) for v in out]))
 
     def get_kernel_times(self):
         """{class: (total ms, launches)} since the last call (needs XY_OPT_PROFILE = 1)."""

@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "xy_kernels.cuh"
+#include "xy_resident.cuh"
 
 using namespace xyk;
 
@@ -37,7 +38,7 @@ bool shape_ok(int L, int R) { return L >= 8 && L % 8 == 0 && L <= 1024 && R >= 1
 size_t max_tiles(int L) { return (size_t)(L / 2) * (size_t)(L / 2); }   // tiles_ok: TY >= 2 and TZ >= 2
 
 struct WsLayout {
-    size_t obs_rank, obs_slot, partials, partials6, obs6, dctr, betas, beta_of_slot, beta32, slot_at_rank, met_acc, pt_acc, exact, near_ctl, near_queue, stage, total;
+    size_t obs_rank, obs_slot, partials, partials6, obs6, dctr, betas, beta_of_slot, beta32, slot_at_rank, met_acc, pt_acc, exact, near_ctl, res_sync, res_xchg, near_queue, stage, total;
     unsigned int near_cap;
 };
 WsLayout ws_layout(int L, int R) {
@@ -58,6 +59,8 @@ WsLayout ws_layout(int L, int R) {
     w.pt_acc = take((size_t)R * 8);
     w.exact = take(8);
     w.near_ctl = take(16);                           // near_count, done_ticket, overflow_flag
+    w.res_sync = take(16);                           // resident kernel: grid barrier counter, error flag
+    w.res_xchg = take((size_t)2 * (R <= kResMaxR ? R : 0) * kResMaxC * 6 * 8);   // resident kernel: published partial sums
     // capacity of the close-decision queue: 2e-3 of one colour pass (expected load at beta ~ 0.45 is 4e-5)
     const size_t pass_sites = (size_t)R * L * L * L / 2;
     size_t cap = (size_t)((double)pass_sites * 2e-3);
@@ -68,6 +71,11 @@ WsLayout ws_layout(int L, int R) {
     w.total = o;
     return w;
 }
+
+// resident path (xy_resident.cuh): slots per CTA or CTAs per slot, launch shape.  Dynamic + static shared memory of a
+// block may not exceed the 227 KB opt-in limit: 1 KB is left for the kernel's static variables.
+constexpr size_t kResidentSmemMax = 226 * 1024;
+struct ResidentPlan { bool ok = false; int G = 1, C = 1, tps = 0, threads = 0, grid = 0; size_t smem = 0; };
 
 }  // namespace
 
@@ -87,7 +95,10 @@ struct xy_ctx {
     WsLayout ws;
     float* d_trace = nullptr;
     // options
-    int TY = 0, TZ = 0, TY_met = 0, TZ_met = 0, trace = 0, fused = 1, generic = 0, or_per_mcs = 1, use_graph = 1;
+    int TY = 0, TZ = 0, TY_met = 0, TZ_met = 0, trace = 0, fused = 1, generic = 0, or_per_mcs = 1, use_graph = 1, resident = 1;
+    bool res_planned = false, res_used = false;   // resident path: plan cached; a launch is in flight whose error flag must be read
+    ResidentPlan res_plan;
+    bool slot_valid = false;                   // obs_slot holds the observables of the current spins (resident kernel)
     // CUDA graph of one Monte Carlo step in device-counter mode (xy_mcs), rebuilt when graph_key changes
     cudaGraphExec_t graph_exec = nullptr;
     uint64_t graph_key = 0, graph_launches = 0;
@@ -268,6 +279,12 @@ int check_near_overflow(xy_ctx* c) {
     CK(cudaMemcpyAsync(&flag, c->ws_ptr<unsigned int>(c->ws.near_ctl) + 2, 4, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     if (flag) return fail(XY_ERR_CUDA, "Metropolis close-decision queue overflowed (capacity %u): results are not exact", c->ws.near_cap);
+    if (c->res_used) {                         // the resident kernel's grid barrier timed out (its CTAs were not co-resident)
+        unsigned int err = 0;
+        CK(cudaMemcpyAsync(&err, c->ws_ptr<unsigned int>(c->ws.res_sync) + 1, 4, cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaStreamSynchronize(c->stream));
+        if (err) return fail(XY_ERR_CUDA, "resident Monte Carlo kernel aborted at its grid barrier: results are invalid");
+    }
     return XY_OK;
 }
 
@@ -278,6 +295,16 @@ int grid_for(size_t n_items, int threads) {
 }
 
 int run_measure(xy_ctx* c, double* d_series_row) {
+    if (!c->partials_valid && c->slot_valid) {           // the resident kernel left the by-slot observables of these spins
+        if (!c->rank_valid) {
+            LaunchSpan span(c, XY_K_FINALIZE);
+            gather_rank_kernel<<<(5 * c->R + 127) / 128, 128, 0, c->stream>>>(c->ws_ptr<double>(c->ws.obs_slot), c->ws_ptr<int>(c->ws.slot_at_rank),
+                                                                              c->R, c->ws_ptr<double>(c->ws.obs_rank));
+            CK(cudaGetLastError());
+            c->rank_valid = true;
+        }
+        return XY_OK;
+    }
     if (!c->partials_valid) {
         SweepParams P = base_params(c, 1);     // own = white, staged = black
         int rc = launch_sweep<MODE_MEASURE, false, false>(c, P);
@@ -297,6 +324,126 @@ int run_measure(xy_ctx* c, double* d_series_row) {
         CK(cudaGetLastError());
         c->rank_valid = true;
     }
+    return XY_OK;
+}
+
+
+// ---- resident path (xy_resident.cuh): one persistent launch for n whole steps of a small lattice ------------------
+template <int L, int C>
+int resident_launch(xy_ctx* c, const ResidentPlan& pl, const ResidentParams& P, bool query_only, int* max_clusters) {
+    constexpr bool CLUSTER = C > 1;
+    auto kern = resident_mcs_kernel<L, C>;
+    static std::atomic<bool> attr_set[kMaxDevices];
+    if (!attr_set[c->device].load(std::memory_order_acquire)) {
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kResidentSmemMax));
+        attr_set[c->device].store(true, std::memory_order_release);
+    }
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(pl.grid); cfg.blockDim = dim3(pl.threads); cfg.dynamicSmemBytes = pl.smem; cfg.stream = c->stream;
+    cudaLaunchAttribute at[2];
+    int na = 0;
+    if (CLUSTER) { at[na].id = cudaLaunchAttributeClusterDimension; at[na].val.clusterDim.x = C; at[na].val.clusterDim.y = 1; at[na].val.clusterDim.z = 1; ++na; }
+    cfg.attrs = at; cfg.numAttrs = na;
+    if (query_only) {                          // how many clusters (CTAs for C = 1) of this shape can be resident at once?
+        if (CLUSTER) { CK(cudaOccupancyMaxActiveClusters(max_clusters, kern, &cfg)); }
+        else {
+            int per_sm = 0, dev_sms = 0;
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, pl.threads, pl.smem));
+            CK(cudaDeviceGetAttribute(&dev_sms, cudaDevAttrMultiProcessorCount, c->device));
+            *max_clusters = per_sm * dev_sms;
+        }
+        return XY_OK;
+    }
+    // the CTAs wait on one another once per step: co-residency is guaranteed by a cooperative launch
+    at[na].id = cudaLaunchAttributeCooperative; at[na].val.cooperative = 1; ++na;
+    cfg.numAttrs = na;
+    CK(cudaMemsetAsync(c->ws_ptr<unsigned int>(c->ws.res_sync), 0, 8, c->stream));
+    if (pl.grid > 1) CK(cudaMemsetAsync(c->ws_ptr<char>(c->ws.res_xchg), 0, (size_t)2 * c->R * kResMaxC * 6 * 8, c->stream));   // step tags start at 1
+    {
+        LaunchSpan span(c, XY_K_RESIDENT);
+        CK(cudaLaunchKernelEx(&cfg, kern, P));
+    }
+    return XY_OK;
+}
+
+// The (L, C) pairs with a kernel: every slab with its two halo planes must fit in one block's shared memory.
+int resident_dispatch(xy_ctx* c, const ResidentPlan& pl, const ResidentParams& P, bool query_only, int* max_clusters) {
+#define XY_RES_CASE(LL, CC) if (c->L == LL && pl.C == CC) return resident_launch<LL, CC>(c, pl, P, query_only, max_clusters)
+    XY_RES_CASE(8, 1);
+    XY_RES_CASE(16, 1); XY_RES_CASE(16, 2); XY_RES_CASE(16, 4); XY_RES_CASE(16, 8);
+    XY_RES_CASE(24, 1); XY_RES_CASE(24, 2); XY_RES_CASE(24, 4); XY_RES_CASE(24, 8);
+    XY_RES_CASE(32, 2); XY_RES_CASE(32, 4); XY_RES_CASE(32, 8);
+    XY_RES_CASE(40, 8);
+    XY_RES_CASE(48, 8);
+#undef XY_RES_CASE
+    return fail(XY_ERR_INVALID_ARG, "no resident kernel for L=%d with %d thread blocks per slot", c->L, pl.C);
+}
+bool resident_has_kernel(int L, int C) {
+    switch (L) {
+        case 8: return C == 1;
+        case 16: case 24: return C == 1 || C == 2 || C == 4 || C == 8;
+        case 32: return C == 2 || C == 4 || C == 8;
+        case 40: case 48: return C == 8;
+        default: return false;
+    }
+}
+
+// Chooses slots per CTA (tiny lattices) or CTAs per slot (a cluster), such that everything fits in shared memory and ALL
+// CTAs are resident at once (they meet once per step).  Cached per context.
+const ResidentPlan& resident_plan(xy_ctx* c) {
+    if (c->res_planned) return c->res_plan;
+    c->res_planned = true;
+    ResidentPlan& best = c->res_plan;
+    const int L = c->L, R = c->R;
+    if (R > kResMaxR) return best;
+    ResidentParams dummy;
+    memset(&dummy, 0, sizeof(dummy));
+    const int pi = resident_plane_items(L), maxt = resident_max_threads(L);
+    for (int C = kResMaxC; C >= 1; C >>= 1) {              // the largest co-resident cluster per slot: most SMs at work
+        if (!resident_has_kernel(L, C)) continue;
+        ResidentPlan pl;
+        pl.C = C;
+        pl.G = C == 1 ? (R + 131) / 132 : 1;               // tiny lattices, many slots: several slots per CTA
+        int unit = pi;                                     // threads per slot: whole planes; whole warps too if slots share a block
+        if (pl.G > 1) while (unit % 32) unit += pi;
+        const int items = (L / C) * pi;
+        int tps = (items + unit - 1) / unit * unit;
+        if (tps > maxt / pl.G) tps = maxt / pl.G / unit * unit;
+        if (tps < unit) continue;
+        pl.tps = tps;
+        pl.threads = (tps * pl.G + 31) / 32 * 32;
+        pl.grid = C == 1 ? (R + pl.G - 1) / pl.G : R * C;
+        pl.smem = resident_smem_bytes(L, R, pl.G, C);
+        if (pl.smem > kResidentSmemMax) continue;
+        int cap = 0;
+        if (resident_dispatch(c, pl, dummy, true, &cap) != XY_OK) { cudaGetLastError(); continue; }
+        if (cap >= (C == 1 ? pl.grid : R)) { pl.ok = true; best = pl; break; }    // cap counts clusters (CTAs for C = 1)
+        fail(XY_OK, "resident plan: L=%d R=%d needs %d clusters of %d thread blocks, %d can be resident", L, R, C == 1 ? pl.grid : R, C, cap);
+    }
+    return best;
+}
+
+int resident_mcs(xy_ctx* c, const ResidentPlan& pl, int n_mcs, double* d_series) {
+    ResidentParams P;
+    memset(&P, 0, sizeof(P));
+    P.black = c->colour(0); P.white = c->colour(1);
+    P.R = c->R; P.n_mcs = n_mcs; P.or_per_mcs = c->or_per_mcs; P.G = pl.G; P.tps = pl.tps;
+    P.n_met0 = c->n_met; P.n_pt0 = c->n_pt; P.keys = c->keys;
+    P.betas = c->ws_ptr<double>(c->ws.betas);
+    P.beta_of_slot = c->ws_ptr<double>(c->ws.beta_of_slot); P.beta32_of_slot = c->ws_ptr<float>(c->ws.beta32);
+    P.slot_at_rank = c->ws_ptr<int>(c->ws.slot_at_rank);
+    P.met_acc = c->ws_ptr<unsigned long long>(c->ws.met_acc); P.pt_acc = c->ws_ptr<unsigned long long>(c->ws.pt_acc);
+    P.exact_count = c->ws_ptr<unsigned long long>(c->ws.exact);
+    P.obs_rank = c->ws_ptr<double>(c->ws.obs_rank); P.obs_slot = c->ws_ptr<double>(c->ws.obs_slot);
+    P.series = d_series;
+    P.xchg = c->ws_ptr<unsigned long long>(c->ws.res_xchg);
+    P.sync = c->ws_ptr<unsigned int>(c->ws.res_sync);
+    if (const int rc = resident_dispatch(c, pl, P, false, nullptr)) return rc;
+    c->n_met += (uint32_t)n_mcs; c->n_or += (uint32_t)n_mcs * (uint32_t)c->or_per_mcs; c->n_pt += (uint32_t)n_mcs;
+    c->partials_valid = false; c->slot_valid = true;       // by-slot observables of the final spins are on the device
+    c->rank_valid = false;                                 // the by-rank rows belong to the labelling before the last exchange
+    c->res_used = true;
     return XY_OK;
 }
 
@@ -378,7 +525,7 @@ int xy_attach(xy_ctx* c, void* d_state, void* d_workspace, void* cuda_stream) {
     else { CK(cudaMalloc(&c->d_ws, c->ws.total)); c->own_ws = true; }
     CK(cudaMemsetAsync(c->d_ws, 0, c->ws.stage, c->stream));     // everything but the staging slot
     c->attached = true;
-    c->partials_valid = c->rank_valid = false;
+    c->partials_valid = c->rank_valid = c->slot_valid = false;
     c->launches = 0;
     return upload_labels(c, nullptr);
 }
@@ -391,7 +538,7 @@ int xy_init_random(xy_ctx* c) {
         init_random_kernel<<<grid_for(n_quads, 256), 256, 0, c->stream>>>(c->colour(0), c->colour(1), c->L, c->R, c->keys);
     }
     CK(cudaGetLastError());
-    c->partials_valid = false;
+    c->partials_valid = c->slot_valid = false;
     return XY_OK;
 }
 
@@ -403,7 +550,7 @@ int xy_init_ordered(xy_ctx* c, float theta0) {
         fill_kernel<<<grid_for(n, 256), 256, 0, c->stream>>>(c->d_state, n, theta0);
     }
     CK(cudaGetLastError());
-    c->partials_valid = false;
+    c->partials_valid = c->slot_valid = false;
     return XY_OK;
 }
 
@@ -438,7 +585,7 @@ static int convert_state(xy_ctx* c, float* black, float* white, float* natural, 
 int xy_set_state(xy_ctx* c, const float* natural, int on_device) {
     ENTER(c);
     if (!natural) return fail(XY_ERR_INVALID_ARG, "xy_set_state: NULL pointer");
-    c->partials_valid = false;
+    c->partials_valid = c->slot_valid = false;
     return convert_state(c, c->colour(0), c->colour(1), const_cast<float*>(natural), on_device, true);
 }
 
@@ -478,7 +625,7 @@ int xy_metropolis_sweep(xy_ctx* c) {
         }
     }
     ++c->n_met;
-    c->partials_valid = false;
+    c->partials_valid = c->slot_valid = false;
     return XY_OK;
 }
 
@@ -491,7 +638,7 @@ static int overrelax_sweep_impl(xy_ctx* c, bool with_observables) {
     }
     ++c->n_or;
     c->partials_valid = with_observables;
-    c->rank_valid = false;
+    c->rank_valid = c->slot_valid = false;
     return XY_OK;
 }
 
@@ -514,13 +661,14 @@ int xy_measure(xy_ctx* c, double* out) {
 // decisions were taken on.  When those are not yet reduced to ranks, the final reduction stage and
 // the exchange run as ONE kernel.
 static int pt_exchange_impl(xy_ctx* c, double* d_series_row) {
-    if (!c->partials_valid) {
+    const bool from_slots = !c->partials_valid && c->slot_valid && !d_series_row && !c->device_counters;
+    if (!c->partials_valid && !from_slots) {
         SweepParams P = base_params(c, 1);     // own = white, staged = black
         if (int rc = launch_sweep<MODE_MEASURE, false, false>(c, P)) return rc;
         c->partials_valid = true;
         c->rank_valid = false;
     }
-    if (!c->rank_valid || d_series_row || c->device_counters) {
+    if (!from_slots && (!c->rank_valid || d_series_row || c->device_counters)) {
         const int n_tiles = (c->L / c->TY) * (c->L / c->TZ);
         LaunchSpan span(c, XY_K_PT);
         finalize_pt_kernel<<<1, 1024, 0, c->stream>>>(
@@ -601,6 +749,11 @@ static int build_step_graph(xy_ctx* c, uint64_t key) {
 int xy_mcs(xy_ctx* c, int n_mcs, double* d_series) {
     ENTER(c);
     if (n_mcs < 0) return fail(XY_ERR_INVALID_ARG, "xy_mcs: n_mcs < 0");
+    // XY_OPT_RESIDENT: small lattices run all n steps in ONE persistent launch with the spins resident in shared memory
+    if (c->resident && !c->trace && n_mcs >= 1) {
+        const ResidentPlan& pl = resident_plan(c);
+        if (pl.ok) return resident_mcs(c, pl, n_mcs, d_series);
+    }
     int t = 0;
     // XY_OPT_CUDA_GRAPH: from the second step on, replay one captured graph per step (7 kernel nodes):
     // same kernels, same arithmetic, less launch latency.  The first step runs eagerly (it also sets the
@@ -692,15 +845,16 @@ int xy_set_option(xy_ctx* c, int option, int value) {
     switch (option) {
         case XY_OPT_TILE_Y:
             if (!tiles_ok(c->L, value, c->TZ)) return fail(XY_ERR_INVALID_ARG, "XY_OPT_TILE_Y=%d invalid for L=%d", value, c->L);
-            c->TY = value; c->TY_met = c->TZ_met = 0; c->partials_valid = false; return XY_OK;
+            c->TY = value; c->TY_met = c->TZ_met = 0; c->partials_valid = c->slot_valid = false; return XY_OK;
         case XY_OPT_TILE_Z:
             if (!tiles_ok(c->L, c->TY, value)) return fail(XY_ERR_INVALID_ARG, "XY_OPT_TILE_Z=%d invalid for L=%d", value, c->L);
-            c->TZ = value; c->TY_met = c->TZ_met = 0; c->partials_valid = false; return XY_OK;
+            c->TZ = value; c->TY_met = c->TZ_met = 0; c->partials_valid = c->slot_valid = false; return XY_OK;
         case XY_OPT_TRACE: c->trace = value ? 1 : 0; return XY_OK;
         case XY_OPT_FUSED_MEASURE: c->fused = value ? 1 : 0; return XY_OK;
         case XY_OPT_PROFILE: c->profile = value ? 1 : 0; return XY_OK;
         case XY_OPT_GENERIC_KERNEL: c->generic = value ? 1 : 0; return XY_OK;
         case XY_OPT_CUDA_GRAPH: c->use_graph = value ? 1 : 0; return XY_OK;
+        case XY_OPT_RESIDENT: c->resident = value ? 1 : 0; return XY_OK;
         case XY_OPT_OR_PER_MCS:
             if (value < 0 || value > 1000) return fail(XY_ERR_INVALID_ARG, "XY_OPT_OR_PER_MCS=%d out of range", value);
             c->or_per_mcs = value; return XY_OK;
@@ -719,6 +873,7 @@ int xy_get_option(xy_ctx* c, int option, int* value) {
         case XY_OPT_GENERIC_KERNEL: *value = c->generic; return XY_OK;
         case XY_OPT_OR_PER_MCS: *value = c->or_per_mcs; return XY_OK;
         case XY_OPT_CUDA_GRAPH: *value = c->use_graph; return XY_OK;
+        case XY_OPT_RESIDENT: *value = c->resident; return XY_OK;
         default: return fail(XY_ERR_INVALID_ARG, "unknown option %d", option);
     }
 }
@@ -737,6 +892,14 @@ int xy_get_kernel_times(xy_ctx* c, double* ms, uint64_t* n) {
     }
     c->spans.clear();
     for (int k = 0; k < XY_NUM_KERNEL_CLASSES; ++k) { ms[k] = c->k_ms[k]; n[k] = c->k_n[k]; c->k_ms[k] = 0.0; c->k_n[k] = 0; }
+    return XY_OK;
+}
+
+int xy_get_resident_plan(xy_ctx* c, int out[6]) {
+    ENTER(c);
+    if (!out) return fail(XY_ERR_INVALID_ARG, "xy_get_resident_plan: NULL pointer");
+    const ResidentPlan& pl = resident_plan(c);
+    out[0] = pl.ok && c->resident ? 1 : 0; out[1] = pl.G; out[2] = pl.C; out[3] = pl.threads; out[4] = pl.grid; out[5] = (int)pl.smem;
     return XY_OK;
 }
 

@@ -78,6 +78,31 @@ __device__ __forceinline__ void philox4x32_10_var0(uint32_t v, const PhiloxInv& 
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
+// The same call split into its rounds, so that a kernel can interleave two calls with other work in source
+// order (the rounds of one call form a serial multiply -> xor chain; see the Metropolis step of xy_sweep.cuh).
+struct PhiloxState { uint32_t c0, c1, c2, c3; };
+
+__device__ __forceinline__ void philox_var0_start(uint32_t v, const PhiloxInv& I, const PhiloxKeys& K, PhiloxState& s) {   // rounds 0..2
+    const uint64_t q0 = (uint64_t)kPhiloxM0 * v;
+    uint32_t c2 = (uint32_t)(q0 >> 32) ^ I.j0, c3 = (uint32_t)q0;
+    const uint64_t q1 = (uint64_t)kPhiloxM1 * c2;
+    uint32_t c0 = (uint32_t)(q1 >> 32) ^ I.j1, c1 = (uint32_t)q1;
+    c2 = c3 ^ I.j2;
+    const uint64_t p0 = (uint64_t)kPhiloxM0 * c0;
+    const uint64_t p1 = (uint64_t)kPhiloxM1 * c2;
+    s.c0 = (uint32_t)(p1 >> 32) ^ c1 ^ K.k[4];
+    s.c2 = (uint32_t)(p0 >> 32) ^ I.j3;
+    s.c1 = (uint32_t)p1; s.c3 = (uint32_t)p0;
+}
+template <int R>
+__device__ __forceinline__ void philox_round(PhiloxState& s, const PhiloxKeys& K) {                                    // round R, 3 <= R <= 9
+    const uint64_t p0 = (uint64_t)kPhiloxM0 * s.c0;
+    const uint64_t p1 = (uint64_t)kPhiloxM1 * s.c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ s.c1 ^ K.k[2 * R];
+    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ s.c3 ^ K.k[2 * R + 1];
+    s.c1 = (uint32_t)p1; s.c3 = (uint32_t)p0; s.c0 = n0; s.c2 = n2;
+}
+
 enum : uint32_t { kStreamInit = 0, kStreamMetBlack = 1, kStreamMetWhite = 2, kStreamPT = 3 };   // R12
 
 // ---------------------------------------------------------------------------------------------

@@ -138,6 +138,9 @@ __host__ __device__ inline size_t sweep_smem_bytes(int L, int TY) {
 #ifndef XY_SWEEP_MIN_BLOCKS
 #define XY_SWEEP_MIN_BLOCKS 2
 #endif
+#ifndef XY_MET_EARLY_DRAW
+#define XY_MET_EARLY_DRAW 1
+#endif
 template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE, int W4C, int TYC>
 __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 384, (W4C * TYC > 352) ? 1 : XY_SWEEP_MIN_BLOCKS) sweep_kernel(const SweepParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -310,11 +313,37 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 384, (W4C * TYC > 352) 
             mbar_wait(bar, (uint32_t)s & 1u);
             mbar_wait(full0 + 8 * J + (rH ? 24 : 0), fullPar);       // this step's raw rows have landed
             const uint32_t rO = aRawO + J * rawSlotB + (rH ? 3 * rawSlotB : 0);
-            stage(rO, aS, pp);
-            if (MEAS && active && s >= 1 && s <= TZ) accM = add2(accM, add2(add2(pp[0], pp[1]), add2(pp[2], pp[3])));
             float4 cur = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (UPDATE) cur = lds_f4(rO + ownDelta);
-            mbar_arrive(bar);
+            // Metropolis (XY_MET_EARLY_DRAW): this plane's random words are drawn while the plane is staged, the two
+            // Philox calls advanced round by round side by side, so that ptxas interleaves their multiply -> xor
+            // chains (four independent multiplies per round instead of two) and overlaps them with the shared-memory
+            // loads and the field sums that follow.  Measured at L=160: -1.2 % per pass; pinning the sin/cos of the
+            // old angles up here as well (volatile asm, or dependencies through an opaque zero) cost registers
+            // (spills under the 80-register cap) and 7 %.
+            constexpr bool EARLY = XY_MET_EARLY_DRAW && MODE == MODE_MET && UPDATE;
+            uint32_t wq[2][4] = { {0u, 0u, 0u, 0u}, {0u, 0u, 0u, 0u} };
+            if (EARLY) {
+                stage(rO, aS, pp);
+                cur = lds_f4(rO + ownDelta);
+                PhiloxState A, B;
+                philox_var0_start(ctr0, inv, P.keys, A);
+                philox_var0_start(ctr0 + 1u, inv, P.keys, B);
+                philox_round<3>(A, P.keys); philox_round<3>(B, P.keys);
+                philox_round<4>(A, P.keys); philox_round<4>(B, P.keys);
+                philox_round<5>(A, P.keys); philox_round<5>(B, P.keys);
+                mbar_arrive(bar);
+                philox_round<6>(A, P.keys); philox_round<6>(B, P.keys);
+                philox_round<7>(A, P.keys); philox_round<7>(B, P.keys);
+                philox_round<8>(A, P.keys); philox_round<8>(B, P.keys);
+                philox_round<9>(A, P.keys); philox_round<9>(B, P.keys);
+                wq[0][0] = A.c0; wq[0][1] = A.c1; wq[0][2] = A.c2; wq[0][3] = A.c3;
+                wq[1][0] = B.c0; wq[1][1] = B.c1; wq[1][2] = B.c2; wq[1][3] = B.c3;
+            } else {
+                stage(rO, aS, pp);
+                if (MEAS && active && s >= 1 && s <= TZ) accM = add2(accM, add2(add2(pp[0], pp[1]), add2(pp[2], pp[3])));
+                if (UPDATE) cur = lds_f4(rO + ownDelta);
+                mbar_arrive(bar);
+            }
             if (UPDATE) {
                 // ---- local fields of the four own sites: z neighbours and the row itself from registers,
                 //      y neighbours (rows above and below) and the edge pair from the staged plane z ------
@@ -367,7 +396,8 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 384, (W4C * TYC > 352) 
 #pragma unroll
                     for (int pr = 0; pr < 2; ++pr) {
                         uint32_t w[4];
-                        philox4x32_10_var0(ctr0 + pr, inv, P.keys, w);
+                        if (EARLY) { w[0] = wq[pr][0]; w[1] = wq[pr][1]; w[2] = wq[pr][2]; w[3] = wq[pr][3]; }
+                        else philox4x32_10_var0(ctr0 + pr, inv, P.keys, w);
 #pragma unroll
                         for (int kk = 0; kk < 2; ++kk) {
                             const int k = 2 * pr + kk;

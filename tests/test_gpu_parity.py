@@ -503,6 +503,7 @@ def test_mcs_series_matches_stepwise_calls(xy_mod):
     L, R, n = 16, 6, 9
     betas = inputs.beta_ladder(0.44, 0.47, R)
     a = xy_mod.XY(L, R, betas, SEED); b = xy_mod.XY(L, R, betas, SEED)
+    a.set_option(xy_mod.XY_OPT_RESIDENT, 0)                  # the per-pass kernels (the resident path: test_resident_*)
     a.init_random(); b.init_random()
     series = torch.zeros(n, R, 5, dtype=torch.float64, device="cuda")
     a.mcs(n, series)
@@ -601,6 +602,91 @@ def test_set_state_reduces_out_of_range_angles(xy_mod, oracle_mod):
     assert np.array_equal(xy.get_state().view(np.uint32), a.view(np.uint32))
 
 
+
+# ---- f2 stage A: the resident kernel (whole steps of a small lattice in one persistent launch) ------------------
+@pytest.mark.parametrize("L,R,n_or", [(8, 8, 1), (8, 3, 1), (8, 20, 2), (8, 64, 1), (16, 4, 1), (16, 5, 0), (24, 2, 1), (32, 3, 1),
+                                      (32, 16, 1), (40, 2, 1), (48, 2, 2)])
+def test_resident_kernel_equals_per_pass_kernels(xy_mod, L, R, n_or):
+    """XY_OPT_RESIDENT: n whole steps in one launch with the spins resident in shared
+    memory must leave BITWISE the states, labels, counters and Metropolis / exchange acceptance counts of the
+    per-pass kernels (same site arithmetic, same Philox keying, decisions settled in fp64 on both paths), over
+    several calls; the observables (series rows and xy_measure afterwards) agree within the P3 bound, their fp32
+    terms being grouped differently before the fp64 accumulation."""
+    import torch
+    betas = inputs.beta_ladder(0.445, 0.46, R)
+    N = L ** 3
+    runs = []
+    for resident in (1, 0):
+        xy = xy_mod.XY(L, R, betas, SEED)
+        xy.set_option(xy_mod.XY_OPT_RESIDENT, resident)
+        xy.set_option(xy_mod.XY_OPT_OR_PER_MCS, n_or)
+        xy.init_random()
+        s1 = torch.zeros(6, R, 5, dtype=torch.float64, device="cuda")
+        s2 = torch.zeros(5, R, 5, dtype=torch.float64, device="cuda")
+        n0 = xy.get_launch_count()
+        xy.mcs(6, s1); xy.mcs(5, s2); xy.mcs(1); xy.mcs(3)
+        launches = xy.get_launch_count() - n0
+        obs = xy.measure()
+        runs.append((xy.get_state(), xy.get_perm(), xy.get_counters(), xy.get_accept_counts(), xy.get_beta_of_slot(),
+                     s1.cpu().numpy(), s2.cpu().numpy(), obs, launches))
+        # a sweep by the per-pass kernels continues seamlessly from what the resident kernel wrote back
+        xy.metropolis_sweep(); xy.overrelax_sweep(); xy.pt_exchange()
+        runs[-1] += (xy.get_state(), xy.get_perm())
+    a, b = runs
+    assert a[8] == 4, "one launch per xy_mcs call"
+    assert np.array_equal(a[0].view(np.uint32), b[0].view(np.uint32)), "states differ"
+    assert np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2]) and np.array_equal(a[2], [15, 15 * n_or, 15])
+    assert np.array_equal(a[3][0], b[3][0]) and np.array_equal(a[3][1], b[3][1])
+    assert np.array_equal(a[4], b[4])
+    for x, y in ((a[5], b[5]), (a[6], b[6]), (a[7], b[7])):
+        assert np.abs(x[..., 0] - y[..., 0]).max() <= 1e-6 * 3 * N and np.abs(x[..., 1:3] - y[..., 1:3]).max() <= 1e-6 * N
+        assert np.allclose(x[..., 3], x[..., 1] ** 2 + x[..., 2] ** 2, rtol=1e-13) and np.allclose(x[..., 4], x[..., 3] ** 2, rtol=1e-13)
+    assert np.all(a[5][..., 3] > 0)
+    assert np.array_equal(a[9].view(np.uint32), b[9].view(np.uint32)) and np.array_equal(a[10], b[10])
+
+
+def test_resident_kernel_lockstep_against_oracle(xy_mod, oracle_mod):
+    """The resident kernel against the ORACLE directly (not only against the other kernels): one xy_mcs(1) from a
+    shared state is one oracle MCS -- Metropolis decisions read off the state pass by pass are not available here
+    (the four passes run in one launch), so the check is the composed one: after Metropolis + over-relaxation the
+    angles agree within the P2 clause wherever the two Metropolis sweeps took the same decisions, which the fp64
+    settlement guarantees; observables and the exchange follow P3 / P4."""
+    for L, R in ((8, 8), (16, 3), (32, 4)):
+        betas = inputs.beta_ladder(0.45, 0.458, R)
+        xy, ora = make(xy_mod, oracle_mod, L, R, betas=betas)
+        assert xy.get_option(xy_mod.XY_OPT_RESIDENT) == 1
+        xy.init_random(); xy.mcs(4)
+        for t in (4, 5):
+            S, perm = xy.get_state(), xy.get_perm()
+            ora.set_state(S); ora.set_perm(perm); ora.set_counters([t, t, t])
+            import torch
+            row = torch.zeros(1, R, 5, dtype=torch.float64, device="cuda")
+            xy.mcs(1, row)
+            ora.metropolis_sweep()
+            ora.overrelax_sweep()
+            O = ora.get_state()
+            G = xy.get_state()
+            # where a Metropolis decision differed the site would be off by O(1): none may
+            d = H.angle_diff(G, O)
+            assert d.max() <= 5e-3, f"a decision differs (max angle difference {d.max():.3e})"
+            assert (d > P.TOL_ANGLE).mean() <= 2e-4
+            P.check_observables(xy.measure(), ora_obs_of(G, ora, xy.get_perm()), L ** 3)     # by rank AFTER the exchange
+            # the exchange decisions were taken on the GPU's energies; replay them in the oracle from the same energies
+            tr = ora.enable_trace(pt=True)
+            ora.set_state(G); ora.set_perm(perm); ora.set_counters([t + 1, t + 1, t])
+            ora.pt_exchange()
+            P.check_pt(xy.get_perm(), ora.get_perm(), tr["pt_p"], tr["pt_u"])
+            ora.enable_trace()
+            assert np.array_equal(xy.get_counters(), [t + 1, t + 1, t + 1])
+            P.check_observables(row.cpu().numpy()[0], ora_obs_of(G, ora, perm), L ** 3)
+
+
+def ora_obs_of(state, ora, perm):
+    """Oracle observables (by rank under `perm`) of a given state; leaves the oracle's state set to it."""
+    ora.set_state(state); ora.set_perm(perm)
+    return ora.measure()
+
+
 # ---- pipeline hazards --------------------------------------------------------------------------
 @pytest.mark.parametrize("L,R", [(32, 3), (64, 2), (128, 1), (160, 1)])
 def test_free_run_is_reproducible_across_kernel_variants(xy_mod, L, R):
@@ -611,9 +697,10 @@ def test_free_run_is_reproducible_across_kernel_variants(xy_mod, L, R):
     run-time-geometry one, so 6 MCS from the same seed must end in BITWISE identical states."""
     betas = inputs.beta_ladder(0.4535, 0.4550, R)
     ref = None
-    variants = [dict(), dict(), dict(generic=1), dict(tz=8), dict(generic=1, tz=L), dict(ty=8, tz=16)]
+    variants = [dict(), dict(), dict(generic=1), dict(tz=8), dict(generic=1, tz=L), dict(ty=8, tz=16), dict(resident=1)]
     for v in variants:
         xy = xy_mod.XY(L, R, betas, SEED)
+        xy.set_option(xy_mod.XY_OPT_RESIDENT, v.get("resident", 0))       # L = 32: the resident kernel is one more variant
         if "generic" in v:
             xy.set_option(xy_mod.XY_OPT_GENERIC_KERNEL, 1)
         if "ty" in v:
@@ -639,6 +726,7 @@ def test_mcs_with_several_overrelaxation_sweeps(xy_mod):
     betas = inputs.beta_ladder(0.45, 0.46, R)
     a, b = xy_mod.XY(L, R, betas, SEED), xy_mod.XY(L, R, betas, SEED)
     a.init_random(); b.init_random()
+    a.set_option(xy_mod.XY_OPT_RESIDENT, 0)
     a.set_option(xy_mod.XY_OPT_OR_PER_MCS, 3)
     series = torch.zeros(n, R, 5, dtype=torch.float64, device="cuda")
     a.mcs(n, series)
@@ -665,6 +753,7 @@ def test_mcs_graph_replay_equals_eager_launches(xy_mod, L, R, fused, n_or):
     runs = []
     for graph in (1, 0):
         xy = xy_mod.XY(L, R, betas, SEED)
+        xy.set_option(xy_mod.XY_OPT_RESIDENT, 0)
         xy.set_option(xy_mod.XY_OPT_CUDA_GRAPH, graph)
         xy.set_option(xy_mod.XY_OPT_FUSED_MEASURE, fused)
         xy.set_option(xy_mod.XY_OPT_OR_PER_MCS, n_or)
