@@ -219,6 +219,8 @@ int xy_debug_get_trace(xy_ctx* ctx, float* natural);
 /* Evaluate the kernels' device math on n DEVICE floats (stream = cudaStream_t or NULL):
  * fast sin/cos of x[i]; fast atan2(y[i], x[i]) in [0, 2pi); Philox words of n counters. */
 int xy_debug_sincos(const float* d_x, float* d_cos, float* d_sin, size_t n, void* cuda_stream);
+/* the fp64 sin / cos of the settlement of close Metropolis decisions, for n DEVICE doubles in [0, 2 pi] */
+int xy_debug_sincos64(const double* d_x, double* d_cos, double* d_sin, size_t n, void* cuda_stream);
 int xy_debug_atan2(const float* d_y, const float* d_x, float* d_phi, size_t n, void* cuda_stream);
 int xy_debug_philox(const uint32_t* d_ctr /* n*4 */, uint32_t key0, uint32_t key1,
                     uint32_t* d_out /* n*4 */, size_t n, void* cuda_stream);

@@ -54,6 +54,7 @@ SIGNATURES = {
     "xy_last_error": (C.c_char_p, []),
     "xy_debug_get_trace": (_i, [_vp, _vp]),
     "xy_debug_sincos": (_i, [_vp, _vp, _vp, _sz, _vp]),
+    "xy_debug_sincos64": (_i, [_vp, _vp, _vp, _sz, _vp]),
     "xy_debug_atan2": (_i, [_vp, _vp, _vp, _sz, _vp]),
     "xy_debug_philox": (_i, [_vp, C.c_uint32, C.c_uint32, _vp, _sz, _vp]),
 }
@@ -278,6 +279,16 @@ def debug_sincos(x):
     c, s = torch.empty_like(d), torch.empty_like(d)
     _check(_lib.xy_debug_sincos(d.data_ptr(), c.data_ptr(), s.data_ptr(), d.numel(),
                                 torch.cuda.current_stream().cuda_stream), "xy_debug_sincos")
+    return c.cpu().numpy(), s.cpu().numpy()
+
+
+def debug_sincos64(x):
+    torch = _torch()
+    load_library()
+    d = torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64)).cuda()
+    c, s = torch.empty_like(d), torch.empty_like(d)
+    _check(_lib.xy_debug_sincos64(d.data_ptr(), c.data_ptr(), s.data_ptr(), d.numel(),
+                                  torch.cuda.current_stream().cuda_stream), "xy_debug_sincos64")
     return c.cpu().numpy(), s.cpu().numpy()
 
 

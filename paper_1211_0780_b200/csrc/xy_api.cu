@@ -928,6 +928,13 @@ int xy_debug_sincos(const float* d_x, float* d_cos, float* d_sin, size_t n, void
     return XY_OK;
 }
 
+int xy_debug_sincos64(const double* d_x, double* d_cos, double* d_sin, size_t n, void* stream) {
+    if (!d_x || !d_cos || !d_sin) return fail(XY_ERR_INVALID_ARG, "xy_debug_sincos64: NULL pointer");
+    debug_sincos64_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)stream>>>(d_x, d_cos, d_sin, n);
+    CK(cudaGetLastError());
+    return XY_OK;
+}
+
 int xy_debug_atan2(const float* d_y, const float* d_x, float* d_phi, size_t n, void* stream) {
     if (!d_x || !d_y || !d_phi) return fail(XY_ERR_INVALID_ARG, "xy_debug_atan2: NULL pointer");
     debug_atan2_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)stream>>>(d_y, d_x, d_phi, n);

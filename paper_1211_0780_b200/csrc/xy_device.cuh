@@ -169,6 +169,37 @@ __device__ __forceinline__ float fast_atan2_pos(float y, float x) {
 //   other: this slot's other-colour array [z][y][W];  par: x parity of this site's row,
 //   xh: x >> 1.  Neighbour order mirrors the definition: -x, -y, -z, +x, +y, +z.
 // ---------------------------------------------------------------------------------------------
+// fp64 sin and cos of an angle in [0, 2 pi] (the range every stored or proposed angle lies in): quadrant reduction with a
+// two-part pi/2, then the Taylor polynomials to r^17 / r^16 on |r| <= pi/4 (truncation 1e-19 / 2e-18, so the result
+// is within ~1.5e-16 of the true value like a libm sincos).  One third of the dependent-operation depth of the
+// general-range library routine: the fp64 settlement of a close decision holds up a whole thread block (resident
+// kernel) for the length of this chain.  Measured against numpy by tests/test_gpu_parity.py::test_device_math_errors.
+__device__ __forceinline__ void sincos_0_2pi(double x, double& s, double& c) {
+    const double kf = rint(x * 0.63661977236758134308);
+    double r = fma(-kf, 1.5707963267948966, x);
+    r = fma(-kf, 6.123233995736766e-17, r);
+    const double z = r * r;
+    double ps = 2.81145725434552060e-15, pc = 4.77947733238738525e-14;
+    ps = fma(ps, z, -7.64716373181981641e-13); pc = fma(pc, z, -1.14707455977297245e-11);
+    ps = fma(ps, z, 1.60590438368216133e-10);  pc = fma(pc, z, 2.08767569878681002e-09);
+    ps = fma(ps, z, -2.50521083854417202e-08); pc = fma(pc, z, -2.75573192239858883e-07);
+    ps = fma(ps, z, 2.75573192239858925e-06);  pc = fma(pc, z, 2.48015873015873016e-05);
+    ps = fma(ps, z, -1.98412698412698413e-04); pc = fma(pc, z, -1.38888888888888894e-03);
+    ps = fma(ps, z, 8.33333333333333322e-03);  pc = fma(pc, z, 4.16666666666666644e-02);
+    ps = fma(ps, z, -1.66666666666666657e-01); pc = fma(pc, z, -5.00000000000000000e-01);
+    const double sr = fma(r * z, ps, r), cr = fma(z, pc, 1.0);
+    const int q = (int)kf;
+    s = (q & 1) ? cr : sr; c = (q & 1) ? sr : cr;
+    if (q & 2) s = -s;
+    if ((q + 1) & 2) c = -c;
+}
+
+// The fp64 acceptance test u < exp(x), x = -beta dE, taken as log(u) < x: the logarithm does not depend on the fields,
+// so it leaves the dependent chain of the settlement (callers compute it early).  Both forms agree except where u and
+// exp(x) differ by a few ulp; u = 0 keeps the exp form (0 < exp(x) fails only when exp underflows to zero).
+__device__ __forceinline__ double accept_log_u(double u) { return u > 0.0 ? log(u) : 0.0; }
+__device__ __forceinline__ bool accept_exact(double u, double log_u, double x) { return u > 0.0 ? log_u < x : exp(x) > 0.0; }
+
 __device__ __noinline__ bool metropolis_exact(const float* __restrict__ other, int L, int W, int par,
                                               int xh, int y, int z, float t_old, float t_new, float u,
                                               float beta32) {
@@ -180,18 +211,19 @@ __device__ __noinline__ bool metropolis_exact(const float* __restrict__ other, i
     const float nb[6] = {
         other[row * W + xm], other[((size_t)z * L + ym) * W + xh], other[((size_t)zm * L + y) * W + xh],
         other[row * W + xp], other[((size_t)z * L + yp) * W + xh], other[((size_t)zp * L + y) * W + xh] };
+    const double lu = accept_log_u((double)u);
     double hx = 0.0, hy = 0.0;
 #pragma unroll 1
     for (int j = 0; j < 6; ++j) {
         double s, c;
-        sincos((double)nb[j], &s, &c);
+        sincos_0_2pi((double)nb[j], s, c);
         hx += c; hy += s;
     }
     double so, co, sn, cn;
-    sincos((double)t_old, &so, &co);
-    sincos((double)t_new, &sn, &cn);
+    sincos_0_2pi((double)t_old, so, co);
+    sincos_0_2pi((double)t_new, sn, cn);
     const double dE = -(hx * (cn - co) + hy * (sn - so));
-    return (double)u < exp(-(double)beta32 * dE);
+    return accept_exact((double)u, lu, -(double)beta32 * dE);
 }
 
 // Half-width of the window around p_fast inside which the decision is re-evaluated in fp64:

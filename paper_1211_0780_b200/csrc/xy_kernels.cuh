@@ -74,7 +74,8 @@ __global__ void __launch_bounds__(256) met_fixup_kernel(const FixupParams F) {
         float a = role == 6 ? t_old : t_new;
         if (role < 6 && live) a = other[((size_t)nz * L + ny) * W + nx];
         double sn_, cs_;
-        sincos((double)a, &sn_, &cs_);
+        sincos_0_2pi((double)a, sn_, cs_);
+        const double lu = accept_log_u((double)u);
         double hx = 0.0, hy = 0.0, co = 0.0, so = 0.0, cn = 0.0, sn = 0.0;
         const int base = lane & ~7;
 #pragma unroll
@@ -84,7 +85,7 @@ __global__ void __launch_bounds__(256) met_fixup_kernel(const FixupParams F) {
         }
         if (live && role == 0) {
             const double dE = -(hx * (cn - co) + hy * (sn - so));
-            const bool acc = (double)u < exp(-(double)F.beta32_of_slot[slot] * dE);
+            const bool acc = accept_exact((double)u, lu, -(double)F.beta32_of_slot[slot] * dE);
             F.own[(size_t)slot * F.half_n + idx] = acc ? t_new : t_old;
             if (acc != fast_acc) atomicAdd(F.met_acc + slot, acc ? 1ull : ~0ull);
         }
@@ -284,6 +285,11 @@ __global__ void convert_kernel(float* __restrict__ natural, float* __restrict__ 
 __global__ void debug_sincos_kernel(const float* x, float* c, float* s, size_t n) {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         float ss, cc; fast_sincos(x[i], ss, cc); c[i] = cc; s[i] = ss;
+    }
+}
+__global__ void debug_sincos64_kernel(const double* x, double* c, double* s, size_t n) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        double ss, cc; sincos_0_2pi(x[i], ss, cc); c[i] = cc; s[i] = ss;
     }
 }
 __global__ void debug_atan2_kernel(const float* y, const float* x, float* phi, size_t n) {

@@ -76,18 +76,19 @@ __device__ __forceinline__ double pt_uniform(int k, uint32_t n_pt, const PhiloxK
 __device__ __noinline__ bool metropolis_exact_resident(const float* thO, int ixm, int iym, int izm, int ixp, int iyp, int izp,
                                                        float t_old, float t_new, float u, float beta32) {
     const float nb[6] = { thO[ixm], thO[iym], thO[izm], thO[ixp], thO[iyp], thO[izp] };
+    const double lu = accept_log_u((double)u);
     double hx = 0.0, hy = 0.0;
 #pragma unroll 1
     for (int j = 0; j < 6; ++j) {
         double s, c;
-        sincos((double)nb[j], &s, &c);
+        sincos_0_2pi((double)nb[j], s, c);
         hx += c; hy += s;
     }
     double so, co, sn, cn;
-    sincos((double)t_old, &so, &co);
-    sincos((double)t_new, &sn, &cn);
+    sincos_0_2pi((double)t_old, so, co);
+    sincos_0_2pi((double)t_new, sn, cn);
     const double dE = -(hx * (cn - co) + hy * (sn - so));
-    return (double)u < exp(-(double)beta32 * dE);
+    return accept_exact((double)u, lu, -(double)beta32 * dE);
 }
 
 enum { RES_MET = 0, RES_OR = 1, RES_MEAS = 2 };
@@ -198,6 +199,7 @@ __global__ void __launch_bounds__(resident_max_threads(L), 1) resident_mcs_kerne
             bl = beta32 * 1.44269504f;
             win24 = (fabsf(beta32) * kWindowPerBeta + kWindowAbs) * 4294967296.0f;
         }
+        unsigned int pend = 0u, pend_w = 0u, pend_p = 0u; float pend_old = 0.f;
         for (int zl = zl0; zl < nz; zl += PR) {
             const int z = z0 + zl;
             const int par = (y + z + c) & 1;
@@ -225,6 +227,7 @@ __global__ void __launch_bounds__(resident_max_threads(L), 1) resident_mcs_kerne
 
             if (mode == RES_MET) {
                 uint32_t w[4];
+                bool closek[2], accf[2]; float told[2];
                 philox4x32_10(ctrq + (uint32_t)(XQ * L) * (uint32_t)z, (uint32_t)slot, n_met,
                               c == 0 ? kStreamMetBlack : kStreamMetWhite, P.keys, w);
 #pragma unroll
@@ -236,25 +239,37 @@ __global__ void __launch_bounds__(resident_max_threads(L), 1) resident_mcs_kerne
                     fast_sincos(tn, sn, cn);
                     const float g = fmaf(hx[k], cn - pc[k], hy[k] * (sn - ps[k]));       // = -dE; (pc, ps) == fast_sincos(old angle)
                     const float pf = fast_ex2(fmaf(bl, g, 32.0f));
-                    bool acc = uf < pf;
-                    if (fabsf(uf - pf) < win24) {
-                        // too close to call in fp32: keep the fast decision for now and queue the site; settle_close()
-                        // re-evaluates it in fp64 after the pass, eight lanes per site (a lone thread doing eight fp64
-                        // sincos here would hold up its whole cluster for ~2000 cycles)
+                    const bool acc = uf < pf;
+                    closek[k] = fabsf(uf - pf) < win24;            // too close to call in fp32 (no branch here: the two sites' chains interleave)
+                    told[k] = tht[k]; accf[k] = acc;
+                    if (acc) { tht[k] = tn; pc[k] = cn; ps[k] = sn; ++nacc; changed = true; }
+                }
+                if (closek[0] | closek[1]) {
+                    // rare (4e-5 of the decisions): the fast decision stands for now; the site is remembered in registers,
+                    // queued after the loop, and settle_close() re-evaluates it in fp64, eight lanes per site.  A second
+                    // close site of the same thread in one pass (probability ~1e-9) is settled on the spot.
+#pragma unroll
+                    for (int k = 0; k < 2; ++k) {
+                        if (!closek[k]) continue;
                         const int xh = 2 * xq + k;
+                        const bool fast_acc = accf[k];
                         ++nexact;
-                        const unsigned int qi = atomicAdd(qcount, 1u);
-                        if (qi < kResQueue) {
-                            queue[qi] = make_uint4((unsigned int)zl | ((unsigned int)y << 8) | ((unsigned int)xh << 16) | ((unsigned int)s << 24) |
-                                                   ((unsigned int)par << 30) | (acc ? 0x80000000u : 0u),
-                                                   __float_as_uint(tht[k]), __float_as_uint(tn), w[2 * k + 1]);
-                        } else {                                   // queue full (never at ordinary beta): settle on the spot
+                        if (pend == 0u) {
+                            pend = 0x40000000u | (unsigned int)zl | ((unsigned int)xh << 8) | ((unsigned int)par << 16) | (fast_acc ? 0x20000u : 0u);
+                            pend_old = told[k]; pend_p = w[2 * k]; pend_w = w[2 * k + 1];
+                        } else {
                             const int ixm = row + (par ? xh : (xh == 0 ? W - 1 : xh - 1)), ixp = row + (par ? (xh + 1 == W ? 0 : xh + 1) : xh);
-                            acc = metropolis_exact_resident(thO, ixm, rym + xh, row - PL + xh, ixp, ryp + xh, row + PL + xh,
-                                                            tht[k], tn, word_to_u24(w[2 * k + 1]), beta32);
+                            const float tn = word_to_angle(w[2 * k]);
+                            const bool acc = metropolis_exact_resident(thO, ixm, rym + xh, row - PL + xh, ixp, ryp + xh, row + PL + xh,
+                                                                       told[k], tn, word_to_u24(w[2 * k + 1]), beta32);
+                            if (acc != fast_acc) {
+                                tht[k] = acc ? tn : told[k];
+                                fast_sincos(tht[k], ps[k], pc[k]);
+                                if (acc) ++nacc; else --nacc;
+                                changed = true;
+                            }
                         }
                     }
-                    if (acc) { tht[k] = tn; pc[k] = cn; ps[k] = sn; ++nacc; changed = true; }
                 }
             } else if (mode == RES_OR) {
 #pragma unroll
@@ -285,6 +300,30 @@ __global__ void __launch_bounds__(resident_max_threads(L), 1) resident_mcs_kerne
                 }
             }
         }
+        if (pend) {
+            const unsigned int qi = atomicAdd(qcount, 1u);
+            const int zl = pend & 0xff, xh = (pend >> 8) & 0xff, par = (pend >> 16) & 1;
+            const bool fast_acc = (pend & 0x20000u) != 0u;
+            if (qi < kResQueue) {
+                queue[qi] = make_uint4((unsigned int)zl | ((unsigned int)y << 8) | ((unsigned int)xh << 16) | ((unsigned int)s << 24) |
+                                       ((unsigned int)par << 30) | (fast_acc ? 0x80000000u : 0u), __float_as_uint(pend_old), pend_p, pend_w);
+            } else {                                               // queue full (never at ordinary beta): settle on the spot
+                const int pb = (zl + 1) * PL, row = pb + oRow;
+                const int ixm = row + (par ? xh : (xh == 0 ? W - 1 : xh - 1)), ixp = row + (par ? (xh + 1 == W ? 0 : xh + 1) : xh);
+                const float tn = word_to_angle(pend_p);
+                const bool acc = metropolis_exact_resident(thO, ixm, pb + oYm - 2 * xq + xh, row - PL + xh, ixp, pb + oYp - 2 * xq + xh, row + PL + xh,
+                                                           pend_old, tn, word_to_u24(pend_w), beta32);
+                if (acc != fast_acc) {
+                    const float tv = acc ? tn : pend_old;
+                    float s32, c32;
+                    fast_sincos(tv, s32, c32);
+                    thC[row + xh] = tv; prC[row + xh] = make_float2(c32, s32);
+                    if (zl == 0) { const int j = offC + (nz + 1) * PL + oRow + xh; th_dn[j] = tv; pr_dn[j] = make_float2(c32, s32); }
+                    if (zl == nz - 1) { const int j = offC + oRow + xh; th_up[j] = tv; pr_up[j] = make_float2(c32, s32); }
+                    if (acc) ++nacc; else --nacc;
+                }
+            }
+        }
     };
 
     // fp64 settlement of the queued close decisions of colour pass c (after a __syncthreads): the definition of
@@ -300,7 +339,7 @@ __global__ void __launch_bounds__(resident_max_threads(L), 1) resident_mcs_kerne
             const uint4 q = liveq ? queue[e] : make_uint4(0u, 0u, 0u, 0u);
             const int zl = q.x & 0xff, yy = (q.x >> 8) & 0xff, xh = (q.x >> 16) & 0xff, sl = (q.x >> 24) & 0x3f, par = (q.x >> 30) & 1;
             const bool fast_acc = (q.x >> 31) != 0u;
-            const float t_old = __uint_as_float(q.y), t_new = __uint_as_float(q.z);
+            const float t_old = __uint_as_float(q.y), t_new = word_to_angle(q.z);
             const float* thO = th + (1 - c) * CS + sl * SL;
             const int pb = (zl + 1) * PL, row = pb + yy * W;
             const int rym = pb + (yy == 0 ? L - 1 : yy - 1) * W, ryp = pb + (yy + 1 == L ? 0 : yy + 1) * W;
@@ -311,7 +350,8 @@ __global__ void __launch_bounds__(resident_max_threads(L), 1) resident_mcs_kerne
             float a = role == 6 ? t_old : t_new;
             if (role < 6 && liveq) a = thO[idx];
             double sn_, cs_;
-            sincos((double)a, &sn_, &cs_);
+            sincos_0_2pi((double)a, sn_, cs_);
+            const double uq = (double)word_to_u24(q.w), lu = accept_log_u(uq);          // independent of the fields: overlaps the sincos
             double hx = 0.0, hy = 0.0, co = 0.0, so = 0.0, cn = 0.0, sn = 0.0;
             const int base = lane & ~7;
 #pragma unroll
@@ -321,7 +361,7 @@ __global__ void __launch_bounds__(resident_max_threads(L), 1) resident_mcs_kerne
             }
             if (liveq && role == 0) {
                 const double dEx = -(hx * (cn - co) + hy * (sn - so));
-                const bool acc = (double)word_to_u24(q.w) < exp(-(double)b32[sl] * dEx);
+                const bool acc = accept_exact(uq, lu, -(double)b32[sl] * dEx);
                 if (acc != fast_acc) {
                     const float tv = acc ? t_new : t_old;
                     float s32, c32;

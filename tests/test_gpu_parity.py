@@ -112,6 +112,14 @@ def test_device_math_errors(xy_mod):
           f" rms {np.sqrt((ec ** 2).mean()):.2e}")
     assert np.abs(ec).max() <= P.EPS_SINCOS and np.abs(es).max() <= P.EPS_SINCOS
     assert abs(ec.mean()) < 1e-7 and abs(es.mean()) < 2e-8      # MUFU.COS carries a -7e-8 mean error
+    # the fp64 sin / cos of the settlement of close decisions (sincos_0_2pi): libm-grade on [0, 2 pi]
+    xd = np.concatenate([rng.random(1 << 20) * 2 * np.pi, x[-70000:].astype(np.float64), np.arange(9) * (np.pi / 4),
+                         np.nextafter(np.arange(1, 9) * (np.pi / 4), 0), np.nextafter(np.arange(1, 9) * (np.pi / 4), 7), [6.2831854820251465]])
+    cd, sd = xy_mod.debug_sincos64(xd)
+    ref_c, ref_s = np.cos(xd.astype(np.longdouble)), np.sin(xd.astype(np.longdouble))
+    e64 = max(float(np.abs(cd - ref_c).max()), float(np.abs(sd - ref_s).max()))
+    print(f"sincos64: max|err| {e64:.3e}")
+    assert e64 <= 2.5e-16
     phi = rng.random(1 << 20) * 2 * np.pi
     r = np.exp(rng.uniform(np.log(1e-6), np.log(6.0), size=phi.size))
     hx, hy = (r * np.cos(phi)).astype(np.float32), (r * np.sin(phi)).astype(np.float32)
