@@ -105,6 +105,7 @@ NCU_PEAK_GBS = 8184.0          # ncu's own denominator for dram % of peak: 3996 
 def config_keys(cfg):
     """The workload description both arms print (the reference arm adds what it sampled)."""
     return {"workload": cfg.name, "L": cfg.L, "R": cfg.R, "beta": [cfg.beta_lo, cfg.beta_hi], "start": cfg.start,
+            "ladder": "geometric in beta (PAPER.md:62 family)" if cfg.name.startswith("paper_") else "linear in beta",
             "state_bytes": 4 * cfg.L ** 3 * cfg.R}
 
 
@@ -239,9 +240,10 @@ def run_ours(args, cfg):
         return
     peak, peak_src = measured_peak_gbs()
     # dominant kernel = the class with the largest device time in the timed region
-    dom = max(("metropolis", "overrelax", "measure"), key=lambda k: ktimes[k][0])
+    dom = max(("metropolis", "overrelax", "measure", "resident"), key=lambda k: ktimes[k][0])
+    # the resident kernel (small lattices) runs all K steps in ONE launch: its algorithmic bytes are those of K whole steps
     per_launch_bytes = {"metropolis": BYTES_PER_UPDATE * N * R / 2, "overrelax": BYTES_PER_UPDATE * N * R / 2,
-                        "measure": 4.0 * N * R}
+                        "measure": 4.0 * N * R, "resident": BYTES_PER_UPDATE * updates_per_step * args.steps}
     kern = {}
     for k, (tot, n) in ktimes.items():
         if n:
@@ -264,10 +266,13 @@ def run_ours(args, cfg):
                      "algorithmic_bytes_per_launch": per_launch_bytes[dom],
                      # the second denominator SURVEY.md 8(d) asks for, labelled: ncu's theoretical DRAM peak, and the
                      # dram throughput % ncu itself reported for this kernel in the committed capture (profiles/)
+                     "note": ("spins resident in shared memory for the whole call (XY_OPT_RESIDENT): no HBM traffic inside the timed region; "
+                              "achieved is the 12 B/update model over time, for comparison with the per-pass kernels") if dom == "resident" else None,
                      "frac_of_ncu_peak": ach / NCU_PEAK_GBS, "ncu_peak": NCU_PEAK_GBS,
                      "ncu_dram_pct_of_peak_sustained_elapsed": NCU_TRAFFIC_BYTES.get(cfg.name, {}).get(dom + "_dram_pct")},
         "hbm_roofline_frac_whole_mcs_of_ncu_peak": units * BYTES_PER_UPDATE / (ms * 1e-3) * 1e-9 / NCU_PEAK_GBS,
         "kernels": kern,
+        "path": xy.get_resident_plan(),
         "kernels_measured": f"second pass of {args.steps} steps with a CUDA-event pair around every launch: {ms_profiled / args.steps:.4f} ms per step",
         "e2e": {"value": e2e_units / (e2e_ms * 1e-3) * 1e-9, "unit": UNIT, "h2d_bytes_per_step": 4 * N * R,
                 "d2h_bytes_per_step": R * 5 * 8 + R * 4, "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps,
@@ -294,6 +299,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="index into BASELINE.json configs (default 4: L=160, R=64)")
+    ap.add_argument("--family", default=None, help="one of the paper's own workload families instead (PAPER.md:62), e.g. paper_L80_R34: "
+                                                  "non-uniform (geometric) ladder; see inputs.PAPER_FAMILIES")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--tile-z", type=int, default=0, help="override the march length (tuning; 0 = library default)")
@@ -302,6 +309,11 @@ def main():
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     cfg = inputs.CONFIGS[args.config]
+    if args.family:                                 # same fields as a Config; the ladder is geometric in beta, not linear
+        fam = inputs.paper_family(args.family)
+        b = inputs.betas_of_family(fam)
+        cfg = inputs.Config(fam.name, fam.L, fam.R, float(b[0]), float(b[-1]), fam.start, fam.mcs, 1)
+        inputs.betas_of = lambda c, _b=b: _b      # every arm of this run uses the family's ladder
     if args.impl == "reference":
         run_reference(args, cfg)
     else:

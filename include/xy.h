@@ -188,6 +188,9 @@ int xy_mcs(xy_ctx* ctx, int n_mcs, double* d_series);
 int xy_get_perm(xy_ctx* ctx, int* slot_at_rank /* R, out */);         /* synchronises */
 int xy_set_perm(xy_ctx* ctx, const int* slot_at_rank /* R, a permutation */);
 int xy_get_beta_of_slot(xy_ctx* ctx, double* beta_of_slot /* R, out */); /* synchronises */
+/* Replaces the temperature ladder (R values, rank order): rank k keeps the slot it holds and gets betas[k].  For
+ * tuning a ladder towards temperature-independent swap acceptance [P:62] from xy_get_accept_counts.  Synchronises. */
+int xy_set_betas(xy_ctx* ctx, const double* betas);
 int xy_get_counters(xy_ctx* ctx, uint32_t counters[3] /* n_met, n_or, n_pt */);
 int xy_set_counters(xy_ctx* ctx, const uint32_t counters[3]);
 /* Accepted Metropolis proposals per SLOT and accepted swaps per pair (k, k+1) since attach;

@@ -41,6 +41,7 @@ SIGNATURES = {
     "xy_get_perm": (_i, [_vp, _pi]),
     "xy_set_perm": (_i, [_vp, _pi]),
     "xy_get_beta_of_slot": (_i, [_vp, _pd]),
+    "xy_set_betas": (_i, [_vp, _pd]),
     "xy_get_counters": (_i, [_vp, _pu32]),
     "xy_set_counters": (_i, [_vp, _pu32]),
     "xy_get_accept_counts": (_i, [_vp, _pu64, _pu64]),
@@ -212,6 +213,12 @@ class XY:
         b = np.empty(self.R, dtype=np.float64)
         _check(_lib.xy_get_beta_of_slot(self._h, _np_ptr(b, C.c_double)), "xy_get_beta_of_slot")
         return b
+
+    def set_betas(self, betas):
+        b = np.ascontiguousarray(betas, dtype=np.float64)
+        if b.shape != (self.R,):
+            raise XYError(f"betas must have shape ({self.R},)")
+        _check(_lib.xy_set_betas(self._h, _np_ptr(b, C.c_double)), "xy_set_betas")
 
     def get_counters(self):
         n = np.empty(3, dtype=np.uint32)

@@ -186,7 +186,7 @@ int launch_sweep_impl(xy_ctx* c, const SweepParams& P) {
 }
 
 // Tile geometry as compile-time constants for the lattice sizes of the paper's workloads
-// (L = 32, 64, 128, 160 with their default tiles); everything else takes the run-time variant of
+// (L = 32, 64, 96, 128, 160 with their default tiles; L = 80 has no tile whose warps are uniform in x parity); everything else takes the run-time variant of
 // the same kernel.  The test hook and the large-|beta| variant are always run-time geometry.
 template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE = false>
 int launch_sweep(xy_ctx* c, const SweepParams& P) {
@@ -194,6 +194,7 @@ int launch_sweep(xy_ctx* c, const SweepParams& P) {
         if (MODE == MODE_MET && P.W4 == 20 && P.TY == 32) return launch_sweep_impl<MODE_MET, false, false, false, 20, 32>(c, P);
         if (P.W4 == 20 && P.TY == 16) return launch_sweep_impl<MODE, false, FUSED, false, 20, 16>(c, P);
         if (P.W4 == 16 && P.TY == 16) return launch_sweep_impl<MODE, false, FUSED, false, 16, 16>(c, P);
+        if (P.W4 == 12 && P.TY == 16) return launch_sweep_impl<MODE, false, FUSED, false, 12, 16>(c, P);
         if (P.W4 == 8 && P.TY == 32) return launch_sweep_impl<MODE, false, FUSED, false, 8, 32>(c, P);
         if (P.W4 == 4 && P.TY == 32) return launch_sweep_impl<MODE, false, FUSED, false, 4, 32>(c, P);
     }
@@ -471,7 +472,18 @@ xy_ctx* xy_create(int L, int R, const double* betas, uint64_t seed) {
     }
     // Measured at L=160: the Metropolis pass is 3 % faster as ONE block of 20 + 1 warps per
     // SM (five compute warps on every scheduler) than as two of 10 + 1; the over-relaxation pass is not.
-    if (L == 160 && c->TY == 16) { c->TY_met = 32; c->TZ_met = 32; }
+    if (L == 160 && c->TY == 16) {
+        c->TY_met = 32; c->TZ_met = L;
+        double best = 1e300;                       // march length for ONE resident block per SM, as in default_tiles
+        for (int t = L; t >= 2; --t) {
+            if (L % t) continue;
+            const long blocks = (long)R * (L / c->TY_met) * (L / t);
+            const double cost = (double)((blocks + 147) / 148) * (t + 1.0);
+            if (cost < best * 0.999) { best = cost; c->TZ_met = t; }
+        }
+    }
+    // L = 96 (a paper size): 16 rows x 12 float4 = 6 whole warps with uniform x parity -> the compile-time variant
+    if (L == 96 && tiles_ok(L, 16, c->TZ)) c->TY = 16;
     return c;
 }
 
@@ -803,6 +815,18 @@ int xy_set_perm(xy_ctx* c, const int* p) {
         seen[p[k]] = 1;
     }
     return upload_labels(c, p);
+}
+
+int xy_set_betas(xy_ctx* c, const double* betas) {
+    ENTER(c);
+    if (!betas) return fail(XY_ERR_INVALID_ARG, "xy_set_betas: NULL pointer");
+    for (int k = 0; k < c->R; ++k)
+        if (!std::isfinite(betas[k])) return fail(XY_ERR_INVALID_ARG, "xy_set_betas: betas[%d] is not finite", k);
+    std::vector<int> perm(c->R);
+    CK(cudaMemcpyAsync(perm.data(), c->ws_ptr<int>(c->ws.slot_at_rank), c->R * 4, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    c->betas.assign(betas, betas + c->R);
+    return upload_labels(c, perm.data());          // rank k keeps its slot and gets the new beta_k
 }
 
 int xy_get_beta_of_slot(xy_ctx* c, double* b) {

@@ -39,6 +39,42 @@ def config(name_or_index):
     raise KeyError(name_or_index)
 
 
+# The paper's own workload families: 34 temperatures in T = [2.1, 2.3] for L = 64, 80, 96, 128 and 13 in
+# T = [2.19, 2.21] for L = 160, "chosen such that the acceptance rate of swaps is independent of the temperatures".  The
+# ladder itself is not printed: the stand-in starts geometric in beta (non-uniform) and ladder.equalise_swap_acceptance
+# moves the inner temperatures until the measured per-pair acceptance is flat.
+PaperFamily = namedtuple("PaperFamily", "name L R T_lo T_hi start mcs")
+PAPER_FAMILIES = (
+    PaperFamily("paper_L64_R34", 64, 34, 2.1, 2.3, "random", 200),
+    PaperFamily("paper_L80_R34", 80, 34, 2.1, 2.3, "random", 200),
+    PaperFamily("paper_L96_R34", 96, 34, 2.1, 2.3, "random", 200),
+    PaperFamily("paper_L128_R34", 128, 34, 2.1, 2.3, "random", 200),
+    PaperFamily("paper_L160_R13", 160, 13, 2.19, 2.21, "random", 200),
+)
+
+
+def paper_family(name):
+    for f in PAPER_FAMILIES:
+        if f.name == name:
+            return f
+    raise KeyError(name)
+
+
+def geometric_beta_ladder(T_lo, T_hi, R):
+    """R inverse temperatures from 1/T_hi up to 1/T_lo, constant RATIO between neighbours (so non-uniform in beta and in T)."""
+    lo, hi = 1.0 / T_hi, 1.0 / T_lo
+    if R == 1:
+        return np.array([lo], dtype=np.float64)
+    k = np.arange(R, dtype=np.float64)
+    b = lo * (hi / lo) ** (k / (R - 1))
+    b[0], b[-1] = lo, hi
+    return b
+
+
+def betas_of_family(fam):
+    return geometric_beta_ladder(fam.T_lo, fam.T_hi, fam.R)
+
+
 def beta_ladder(beta_lo, beta_hi, R):
     """beta_k = lo + k (hi - lo)/(R-1), k = 0..R-1, in double, inclusive ends."""
     if R == 1:

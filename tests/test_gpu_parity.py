@@ -524,6 +524,34 @@ def test_mcs_series_matches_stepwise_calls(xy_mod):
 
 
 # ---- full-size configs, sampled (the launch configuration bench.py times) -----------------------
+def sampled_slots_lockstep(xy, ora, name, slots, times):
+    """A free-running GPU trajectory; at every MCS in `times` the oracle re-does Metropolis and over-relaxation for the
+    sampled slots (every site of those slots), and the reduction + exchange for all slots."""
+    L = xy.L
+    t = 0
+    for s_t in times:
+        xy.mcs(s_t - t)
+        t = s_t
+        assert np.array_equal(xy.get_counters(), [t, t, t])
+        S, perm = xy.get_state(), xy.get_perm()
+        stats = metropolis_lockstep(xy, ora, S, t, slots=slots)
+        print(name, "MCS", t, "metropolis", stats)
+        S1 = xy.get_state()
+        del S
+        stats, S2 = overrelax_lockstep(xy, ora, S1, slots=slots)
+        print(name, "MCS", t, "overrelax", stats)
+        del S1
+        ora.set_active_slots(None)
+        ora.set_state(S2); ora.set_perm(perm); ora.set_counters([t + 1, t + 1, t]); xy.set_counters([t + 1, t + 1, t])
+        del S2
+        print(name, "MCS", t, "measure", P.check_observables(xy.measure(), ora.measure(), L ** 3))
+        tr = ora.enable_trace(pt=True)
+        xy.pt_exchange(); ora.pt_exchange()
+        print(name, "MCS", t, "pt", P.check_pt(xy.get_perm(), ora.get_perm(), tr["pt_p"], tr["pt_u"]))
+        ora.enable_trace()
+        t += 1
+
+
 @pytest.mark.parametrize("idx,slots", [(3, (0, 17, 31)), (4, (0, 37, 63))])
 def test_full_size_configs_sampled_slots(xy_mod, oracle_mod, idx, slots):
     """BASELINE.json configs 4 and 5 at full size and full length on the GPU with the default tiling (the
@@ -545,28 +573,56 @@ def test_full_size_configs_sampled_slots(xy_mod, oracle_mod, idx, slots):
         xy.init_ordered(0.0)
     # MCS 3 (just after the start), T/2 and T-1 of the stated 500: the late samples compare an equilibrated
     # state (small-|h| sites, acceptance ~0.55), not only the easy regime right after an ordered start
-    t = 0
-    for s_t in (3, cfg.mcs // 2, cfg.mcs - 1):
-        xy.mcs(s_t - t)
-        t = s_t
-        assert np.array_equal(xy.get_counters(), [t, t, t])
-        S, perm = xy.get_state(), xy.get_perm()
-        stats = metropolis_lockstep(xy, ora, S, t, slots=slots)
-        print(cfg.name, "MCS", t, "metropolis", stats)
-        S1 = xy.get_state()
-        del S
-        stats, S2 = overrelax_lockstep(xy, ora, S1, slots=slots)
-        print(cfg.name, "MCS", t, "overrelax", stats)
-        del S1
-        ora.set_active_slots(None)
-        ora.set_state(S2); ora.set_perm(perm); ora.set_counters([t + 1, t + 1, t]); xy.set_counters([t + 1, t + 1, t])
-        del S2
-        print(cfg.name, "MCS", t, "measure", P.check_observables(xy.measure(), ora.measure(), L ** 3))
-        tr = ora.enable_trace(pt=True)
-        xy.pt_exchange(); ora.pt_exchange()
-        print(cfg.name, "MCS", t, "pt", P.check_pt(xy.get_perm(), ora.get_perm(), tr["pt_p"], tr["pt_u"]))
-        ora.enable_trace()
-        t += 1
+    sampled_slots_lockstep(xy, ora, cfg.name, slots, (3, cfg.mcs // 2, cfg.mcs - 1))
+
+
+# ---- f3: the paper's own workload families and ladders ----------------------------------------------------
+@pytest.mark.parametrize("name,slots", [("paper_L64_R34", None), ("paper_L80_R34", (0, 16, 33)), ("paper_L96_R34", (5, 33)),
+                                        ("paper_L160_R13", (0, 6, 12))])
+def test_paper_families_lockstep(xy_mod, oracle_mod, name, slots):
+    """L = 64 ... 160 with R = 34 temperatures in T = [2.1, 2.3] (R = 13 in [2.19, 2.21] at
+    L = 160) on a NON-uniform (geometric) ladder: a free-running GPU trajectory, re-done by the oracle at MCS 0, 1 and 6
+    (whole system at L = 64, sampled slots above) -- Metropolis, over-relaxation, reduction and exchange."""
+    fam = inputs.paper_family(name)
+    betas = inputs.betas_of_family(fam)
+    xy, ora = make(xy_mod, oracle_mod, fam.L, fam.R, betas=betas)
+    xy.init_random()
+    if slots is None:
+        t = 0
+        for s_t in (0, 1, 6):
+            xy.mcs(s_t - t)
+            t = s_t
+            mcs_lockstep(xy, ora, t)
+            t += 1
+    else:
+        sampled_slots_lockstep(xy, ora, name, slots, (0, 1, 6))
+    assert np.array_equal(xy.get_beta_of_slot()[xy.get_perm()], betas)
+
+
+def test_ladder_equalises_the_swap_acceptance(xy_mod):
+    """P:62 "chosen such that the acceptance rate of swaps is independent of the temperatures": starting from the
+    geometric ladder over a range that straddles T_c, ladder.equalise_swap_acceptance (host arithmetic on
+    xy_get_accept_counts, new ladder through xy_set_betas) must flatten the measured per-pair acceptance while keeping
+    both end temperatures; xy_set_betas must leave the permutation and the spins alone."""
+    from paper_1211_0780_b200 import ladder
+    L, R = 16, 12
+    b0 = inputs.geometric_beta_ladder(1.9, 2.6, R)
+    xy = xy_mod.XY(L, R, b0, SEED)
+    xy.init_random()
+    xy.mcs(300)
+    perm, S = xy.get_perm(), xy.get_state()
+    xy.set_betas(b0 * 1.0)
+    assert np.array_equal(xy.get_perm(), perm) and np.array_equal(xy.get_state().view(np.uint32), S.view(np.uint32))
+    assert np.array_equal(xy.get_beta_of_slot()[perm], b0)
+    b, hist = ladder.equalise_swap_acceptance(xy, b0, rounds=8, n_mcs=1500, burn=200)
+    first, last = hist[0], hist[-1]
+    print("acceptance per pair, geometric ladder:", np.round(first, 3).tolist())
+    print("acceptance per pair, tuned ladder:    ", np.round(last, 3).tolist())
+    print("tuned betas:", np.round(b, 5).tolist())
+    assert b[0] == b0[0] and b[-1] == b0[-1] and np.all(np.diff(b) > 0)
+    assert np.array_equal(xy.get_beta_of_slot()[xy.get_perm()], b)
+    assert (last.max() - last.min()) < 0.5 * (first.max() - first.min())
+    assert last.min() > first.min()
 
 
 @pytest.mark.parametrize("L,R", [(200, 2), (256, 1), (8, 64), (16, 200)])
