@@ -147,15 +147,17 @@ void default_tiles(int L, int R, int& TY, int& TZ) {
     TY = 2;                                        // L up to 1024: TY * L/8 must stay within 11 compute warps
     for (int t = 2; t <= L; ++t)
         if (L % t == 0 && t * W4 <= 320) TY = t;
-    // March length: a block costs TZ + 2 steps (two of them only stage) and 2 blocks fit an SM, so
-    // the pass takes about ceil(blocks / (2 * 148 SMs)) * (TZ + 1) step-times: take the divisor of L
-    // that minimises it (the last, partly filled wave is what a long march wastes).
+    // March length: a block costs TZ + 2 steps (two of them only stage) plus the latency of its first copies (about
+    // 1.5 step-times), and 2 blocks fit an SM.  With w = blocks / (2 * 148 SMs) "waves" the pass takes about
+    // (max(w, 1/2) + 0.3) * (TZ + 3.5) step-times: blocks end at different times, so a fraction of a wave is lost at the
+    // end, not a whole one, and an SM that holds one block instead of two runs it faster.  Take the divisor of L that
+    // minimises it.  Fitted to the measured march-length sweeps at L = 64, 128, 160 (profiles/r2_experiments.md).
     TZ = L;
     double best = 1e300;
     for (int t = L; t >= 2; --t) {
         if (L % t) continue;
-        const long blocks = (long)R * (L / TY) * (L / t);
-        const double cost = (double)((blocks + 295) / 296) * (t + 1.0);
+        const double w = (double)((long)R * (L / TY) * (L / t)) / 296.0;
+        const double cost = (std::fmax(w, 0.5) + 0.3) * (t + 3.5);
         if (cost < best * 0.999) { best = cost; TZ = t; }
     }
 }
