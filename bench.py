@@ -182,6 +182,8 @@ def run_ours(args, cfg):
         xy.set_option(binding.XY_OPT_TILE_Z, args.tile_z)
     if args.generic_kernel:
         xy.set_option(binding.XY_OPT_GENERIC_KERNEL, 1)
+    if args.slot_chunk:
+        xy.set_option(binding.XY_OPT_SLOT_CHUNK, args.slot_chunk)
     def barrier():
         if world > 1:
             dist.barrier()
@@ -258,7 +260,8 @@ def run_ours(args, cfg):
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": dict(config_keys(cfg), l2=f"inputs larger than L2 (state {4 * N * R / 1e9:.2f} GB >> 126 MB)" if 4 * N * R > 4e8
                    else "state fits in L2; no flush", parallelism="replicas only" if world > 1 else "1 GPU",
-                   tile_y=xy.get_option(binding.XY_OPT_TILE_Y), tile_z=xy.get_option(binding.XY_OPT_TILE_Z)),
+                   tile_y=xy.get_option(binding.XY_OPT_TILE_Y), tile_z=xy.get_option(binding.XY_OPT_TILE_Z),
+                   slot_chunk=xy.get_option(binding.XY_OPT_SLOT_CHUNK)),
         "site_mcs_per_ns": units / 2 / (ms * 1e-3) * 1e-9,
         "hbm_roofline_frac_whole_mcs": units * BYTES_PER_UPDATE / (ms * 1e-3) * 1e-9 / peak,
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
@@ -306,6 +309,8 @@ def main():
     ap.add_argument("--tile-z", type=int, default=0, help="override the march length (tuning; 0 = library default)")
     ap.add_argument("--tile-y", type=int, default=0, help="override the tile rows (tuning; 0 = library default)")
     ap.add_argument("--generic-kernel", action="store_true", help="force the run-time-geometry colour-pass kernel (tuning)")
+    ap.add_argument("--slot-chunk", type=int, default=0, help="XY_OPT_SLOT_CHUNK: run the colour passes of K slots at a time back to back "
+                                                          "(L2-resident schedule, SURVEY 8(f) f2; 0 = library default: all slots per pass)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     cfg = inputs.CONFIGS[args.config]

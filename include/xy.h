@@ -63,10 +63,15 @@ enum {
                               P:43 "after several sweeps": microcanonical sweeps are cheap decorrelation) */
     XY_OPT_CUDA_GRAPH = 8, /* 1 (default): xy_mcs replays one captured CUDA graph per step from its second
                               step on (counters live on the device); 0: every kernel is launched eagerly  */
-    XY_OPT_RESIDENT = 9    /* 1 (default): for small lattices (L = 8 ... 48, R <= 512, everything co-resident) xy_mcs
+    XY_OPT_RESIDENT = 9,   /* 1 (default): for small lattices (L = 8 ... 48, R <= 512, everything co-resident) xy_mcs
                               runs all its steps in ONE persistent launch with the spins resident in shared
                               memory (same results: states, labels and counters bitwise, observables
                               within the reduction's rounding); 0: always the per-pass kernels                 */
+    XY_OPT_SLOT_CHUNK = 10 /* K > 0: xy_mcs runs the four colour passes of K slots at a time back to back (launches
+                              over slots [0,K), [K,2K), ...) so that a chunk's spins stay in the 126 MB L2 between
+                              its passes: 8 instead of 24 B of HBM traffic per site and step (SURVEY 8(f) f2 for
+                              lattices too large for shared memory).  Same kernels, bitwise the same results.
+                              0 (default): every pass runs over all slots at once (faster: DESIGN.md section 6) */
 };
 
 /* Kernel classes reported by xy_get_kernel_times. */

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libxy_b200.so")
 _lib = None
 
-XY_OPT_TILE_Y, XY_OPT_TILE_Z, XY_OPT_TRACE, XY_OPT_FUSED_MEASURE, XY_OPT_PROFILE, XY_OPT_GENERIC_KERNEL, XY_OPT_OR_PER_MCS, XY_OPT_CUDA_GRAPH, XY_OPT_RESIDENT = 1, 2, 3, 4, 5, 6, 7, 8, 9
+XY_OPT_TILE_Y, XY_OPT_TILE_Z, XY_OPT_TRACE, XY_OPT_FUSED_MEASURE, XY_OPT_PROFILE, XY_OPT_GENERIC_KERNEL, XY_OPT_OR_PER_MCS, XY_OPT_CUDA_GRAPH, XY_OPT_RESIDENT, XY_OPT_SLOT_CHUNK = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
 KERNEL_CLASSES = ("metropolis", "overrelax", "measure", "finalize", "pt", "other", "fixup", "resident")
 NUM_OBS = 5
 

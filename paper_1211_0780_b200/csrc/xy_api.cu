@@ -2,6 +2,7 @@
 // Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -shared -Xcompiler -fPIC
 #include "../../include/xy.h"
 
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdarg>
@@ -95,7 +96,7 @@ struct xy_ctx {
     WsLayout ws;
     float* d_trace = nullptr;
     // options
-    int TY = 0, TZ = 0, TY_met = 0, TZ_met = 0, trace = 0, fused = 1, generic = 0, or_per_mcs = 1, use_graph = 1, resident = 1;
+    int TY = 0, TZ = 0, TY_met = 0, TZ_met = 0, trace = 0, fused = 1, generic = 0, or_per_mcs = 1, use_graph = 1, resident = 1, slot_chunk = 0;
     bool res_planned = false, res_used = false;   // resident path: plan cached; a launch is in flight whose error flag must be read
     ResidentPlan res_plan;
     bool slot_valid = false;                   // obs_slot holds the observables of the current spins (resident kernel)
@@ -178,7 +179,7 @@ int launch_sweep_impl(xy_ctx* c, const SweepParams& P) {
     }
     const size_t smem = sweep_smem_bytes(P.L, P.TY);
     const int threads = (P.nItems + 31) / 32 * 32 + 32;          // compute warps + the auxiliary warp
-    dim3 grid(P.nTY * P.nTZ, c->R);
+    dim3 grid(P.nTY * P.nTZ, P.n_slots);
     {
         LaunchSpan span(c, MODE == MODE_MET ? XY_K_METROPOLIS : MODE == MODE_OR ? XY_K_OVERRELAX : XY_K_MEASURE);   // MODE_STIFF counts as measure
         sweep_kernel<MODE, TRACE, FUSED, EXACT_INLINE, W4C, TYC><<<grid, threads, smem, c->stream>>>(P);
@@ -221,6 +222,7 @@ SweepParams base_params(xy_ctx* c, int colour) {
     P.L = c->L; P.W = c->L / 2; P.W4 = c->L / 8;
     P.TY = c->TY; P.TZ = c->TZ; P.nTY = c->L / c->TY; P.nTZ = c->L / c->TZ;          // xy_metropolis_sweep may override (TY_met)
     P.colour = colour;
+    P.slot0 = 0; P.n_slots = c->R;                   // all slots; the chunked schedule of xy_mcs narrows them
     P.nItems = P.TY * P.W4;
     P.half_n = (unsigned int)c->half_n;
     P.keys = c->keys;
@@ -609,11 +611,12 @@ int xy_get_state(xy_ctx* c, float* natural, int on_device) {
     return convert_state(c, c->colour(0), c->colour(1), natural, on_device, false);
 }
 
-int xy_metropolis_sweep(xy_ctx* c) {
-    ENTER(c);
+// Both colour passes of one Metropolis sweep over the slots [slot0, slot0 + n_slots); the caller advances n_met.
+static int metropolis_slots(xy_ctx* c, int slot0, int n_slots) {
     if (c->trace && !c->d_trace) CK(cudaMalloc(&c->d_trace, (size_t)c->R * c->N * 4));
     for (int colour = 0; colour < 2; ++colour) {
         SweepParams P = base_params(c, colour);
+        P.slot0 = slot0; P.n_slots = n_slots;
         if (c->TY_met && !c->trace && !c->generic && !need_inline_exact(c)) {
             P.TY = c->TY_met; P.TZ = c->TZ_met; P.nTY = c->L / P.TY; P.nTZ = c->L / P.TZ; P.nItems = P.TY * P.W4;
         }
@@ -638,18 +641,31 @@ int xy_metropolis_sweep(xy_ctx* c) {
             CK(cudaGetLastError());
         }
     }
+    return XY_OK;
+}
+
+int xy_metropolis_sweep(xy_ctx* c) {
+    ENTER(c);
+    if (int rc = metropolis_slots(c, 0, c->R)) return rc;
     ++c->n_met;
     c->partials_valid = c->slot_valid = false;
     return XY_OK;
 }
 
-static int overrelax_sweep_impl(xy_ctx* c, bool with_observables) {
+// Both colour passes of one over-relaxation sweep over the slots [slot0, slot0 + n_slots); the caller advances n_or.
+static int overrelax_slots(xy_ctx* c, bool with_observables, int slot0, int n_slots) {
     for (int colour = 0; colour < 2; ++colour) {
         SweepParams P = base_params(c, colour);
+        P.slot0 = slot0; P.n_slots = n_slots;
         const bool fuse = with_observables && colour == 1;      // the white pass sees the final black sites
         int rc = fuse ? launch_sweep<MODE_OR, false, true>(c, P) : launch_sweep<MODE_OR, false, false>(c, P);
         if (rc) return rc;
     }
+    return XY_OK;
+}
+
+static int overrelax_sweep_impl(xy_ctx* c, bool with_observables) {
+    if (int rc = overrelax_slots(c, with_observables, 0, c->R)) return rc;
     ++c->n_or;
     c->partials_valid = with_observables;
     c->rank_valid = c->slot_valid = false;
@@ -730,6 +746,21 @@ int xy_pt_exchange(xy_ctx* c) {
 
 // One Monte Carlo step enqueued on the stream [P:30].
 static int enqueue_mcs(xy_ctx* c, double* d_series_row) {
+    // XY_OPT_SLOT_CHUNK: all colour passes of K slots back to back, chunk after chunk, so that a chunk's spins are still in
+    // L2 when its next pass reads them.  The passes of different slots are independent (only the
+    // exchange couples replicas), every kernel reads the same step counters: bitwise the same results.
+    if (c->slot_chunk > 0 && c->slot_chunk < c->R && !c->trace) {
+        for (int s0 = 0; s0 < c->R; s0 += c->slot_chunk) {
+            const int n = std::min(c->slot_chunk, c->R - s0);
+            if (int rc = metropolis_slots(c, s0, n)) return rc;
+            for (int j = 0; j < c->or_per_mcs; ++j)
+                if (int rc = overrelax_slots(c, c->fused != 0 && j + 1 == c->or_per_mcs, s0, n)) return rc;
+        }
+        ++c->n_met; c->n_or += (uint32_t)c->or_per_mcs;
+        c->partials_valid = c->fused != 0 && c->or_per_mcs >= 1;
+        c->rank_valid = c->slot_valid = false;
+        return pt_exchange_impl(c, d_series_row);
+    }
     if (int rc = xy_metropolis_sweep(c)) return rc;
     for (int j = 0; j < c->or_per_mcs; ++j)          // only the last sweep's white pass carries the observables
         if (int rc = overrelax_sweep_impl(c, c->fused != 0 && j + 1 == c->or_per_mcs)) return rc;
@@ -776,7 +807,7 @@ int xy_mcs(xy_ctx* c, int n_mcs, double* d_series) {
         if (int rc = enqueue_mcs(c, d_series)) return rc;
         t = 1;
         const uint64_t key = 1u | ((uint64_t)c->TY << 1) ^ ((uint64_t)c->TZ << 12) ^ ((uint64_t)c->fused << 23) ^ ((uint64_t)c->generic << 24) ^
-                             ((uint64_t)c->or_per_mcs << 25) ^ ((uint64_t)c->TY_met << 44) ^ ((uint64_t)need_inline_exact(c) << 36) ^ ((uint64_t)(uintptr_t)c->stream << 37);
+                             ((uint64_t)c->or_per_mcs << 25) ^ ((uint64_t)c->slot_chunk << 50) ^ ((uint64_t)c->TY_met << 44) ^ ((uint64_t)need_inline_exact(c) << 36) ^ ((uint64_t)(uintptr_t)c->stream << 37);
         if (!c->graph_exec || c->graph_key != key)
             if (int rc = build_step_graph(c, key)) return rc;
         DeviceCounters v;
@@ -881,6 +912,9 @@ int xy_set_option(xy_ctx* c, int option, int value) {
         case XY_OPT_GENERIC_KERNEL: c->generic = value ? 1 : 0; return XY_OK;
         case XY_OPT_CUDA_GRAPH: c->use_graph = value ? 1 : 0; return XY_OK;
         case XY_OPT_RESIDENT: c->resident = value ? 1 : 0; return XY_OK;
+        case XY_OPT_SLOT_CHUNK:
+            if (value < 0) return fail(XY_ERR_INVALID_ARG, "XY_OPT_SLOT_CHUNK=%d out of range", value);
+            c->slot_chunk = value; return XY_OK;
         case XY_OPT_OR_PER_MCS:
             if (value < 0 || value > 1000) return fail(XY_ERR_INVALID_ARG, "XY_OPT_OR_PER_MCS=%d out of range", value);
             c->or_per_mcs = value; return XY_OK;
@@ -900,6 +934,7 @@ int xy_get_option(xy_ctx* c, int option, int* value) {
         case XY_OPT_OR_PER_MCS: *value = c->or_per_mcs; return XY_OK;
         case XY_OPT_CUDA_GRAPH: *value = c->use_graph; return XY_OK;
         case XY_OPT_RESIDENT: *value = c->resident; return XY_OK;
+        case XY_OPT_SLOT_CHUNK: *value = c->slot_chunk; return XY_OK;
         default: return fail(XY_ERR_INVALID_ARG, "unknown option %d", option);
     }
 }

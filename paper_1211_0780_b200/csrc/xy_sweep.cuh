@@ -40,6 +40,7 @@ struct SweepParams {
     int L, W, W4;                // W = L/2 floats per row, W4 = L/8 float4 per row
     int TY, TZ, nTY, nTZ;        // tile rows, march length, tiles per replica in y and z
     int colour;                  // colour of `own`
+    int slot0, n_slots;          // this launch covers the slots [slot0, slot0 + n_slots): blockIdx.y = 0 is slot slot0 (XY_OPT_SLOT_CHUNK)
     int nItems;                  // TY * W4 own float4 per plane (<= blockDim.x)
     unsigned int half_n;         // L^3 / 2 floats per slot per colour
     PhiloxKeys keys;
@@ -162,7 +163,7 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 384, (W4C * TYC > 352) 
     const uint32_t full0 = bar + 8;
 
     const int tid = threadIdx.x;
-    const int slot = blockIdx.y;
+    const int slot = blockIdx.y + P.slot0;
     const int tile = blockIdx.x;
     const int tzi = tile / P.nTY, tyi = tile - tzi * P.nTY;
     const int y0 = tyi * TY, z0 = tzi * TZ;

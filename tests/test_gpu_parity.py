@@ -782,6 +782,33 @@ def test_free_run_is_reproducible_across_kernel_variants(xy_mod, L, R):
         assert np.allclose(obs[:, :3], ref[2][:, :3], rtol=0, atol=1e-6 * 3 * L ** 3), v
 
 
+@pytest.mark.parametrize("L,R,chunk,n_or", [(32, 5, 2, 1), (64, 3, 1, 2), (160, 3, 2, 1)])
+def test_slot_chunk_schedule_equals_default(xy_mod, L, R, chunk, n_or):
+    """XY_OPT_SLOT_CHUNK (SURVEY 8(f) f2 for large lattices: the four colour passes of K slots back to back, so that
+    they stay in L2) reorders launches over independent slots only: states, labels, counters and acceptance counts
+    must be bitwise those of the default schedule, the observables equal (same kernels, same tiles), under graph
+    replay and with eager launches."""
+    import torch
+    betas = inputs.beta_ladder(0.45, 0.458, R)
+    out = []
+    for k, graph in ((0, 1), (chunk, 1), (chunk, 0)):
+        xy = xy_mod.XY(L, R, betas, SEED)
+        xy.set_option(xy_mod.XY_OPT_RESIDENT, 0)
+        xy.set_option(xy_mod.XY_OPT_OR_PER_MCS, n_or)
+        xy.set_option(xy_mod.XY_OPT_SLOT_CHUNK, k)
+        xy.set_option(xy_mod.XY_OPT_CUDA_GRAPH, graph)
+        xy.init_random()
+        series = torch.zeros(5, R, 5, dtype=torch.float64, device="cuda")
+        xy.mcs(5, series)
+        out.append((xy.get_state(), xy.get_perm(), xy.get_counters(), xy.get_accept_counts(), series.cpu().numpy(), xy.measure()))
+    ref = out[0]
+    for o in out[1:]:
+        assert np.array_equal(o[0].view(np.uint32), ref[0].view(np.uint32))
+        assert np.array_equal(o[1], ref[1]) and list(o[2]) == list(ref[2])
+        assert np.array_equal(o[3][0], ref[3][0]) and np.array_equal(o[3][1], ref[3][1])
+        assert np.array_equal(o[4], ref[4]) and np.array_equal(o[5], ref[5])
+
+
 def test_mcs_with_several_overrelaxation_sweeps(xy_mod):
     """XY_OPT_OR_PER_MCS: xy_mcs must equal the same calls made one by one, bit for bit, and its
     series rows must be the observables of the state the last over-relaxation sweep left behind."""
