@@ -143,12 +143,19 @@ struct LaunchSpan {
     }
 };
 
+void default_tiles_z(int L, int R, int TY, int& TZ);
+
 void default_tiles(int L, int R, int& TY, int& TZ) {
     const int W4 = L / 8;
     TY = 2;                                        // L up to 1024: TY * L/8 must stay within 11 compute warps
     for (int t = 2; t <= L; ++t)
         if (L % t == 0 && t * W4 <= 320) TY = t;
-    // March length: a block costs TZ + 2 steps (two of them only stage) plus the latency of its first copies (about
+    default_tiles_z(L, R, TY, TZ);
+}
+
+// March length for tile rows TY.
+void default_tiles_z(int L, int R, int TY, int& TZ) {
+    // A block costs TZ + 2 steps (two of them only stage) plus the latency of its first copies (about
     // 1.5 step-times), and 2 blocks fit an SM.  With w = blocks / (2 * 148 SMs) "waves" the pass takes about
     // (max(w, 1/2) + 0.3) * (TZ + 3.5) step-times: blocks end at different times, so a fraction of a wave is lost at the
     // end, not a whole one, and an SM that holds one block instead of two runs it faster.  Take the divisor of L that
@@ -189,7 +196,7 @@ int launch_sweep_impl(xy_ctx* c, const SweepParams& P) {
 }
 
 // Tile geometry as compile-time constants for the lattice sizes of the paper's workloads
-// (L = 32, 64, 96, 128, 160 with their default tiles; L = 80 has no tile whose warps are uniform in x parity); everything else takes the run-time variant of
+// (L = 32, 64, 80, 96, 128, 160 with their default tiles; at L = 80 no tile has warps of uniform x parity: geometry only); everything else takes the run-time variant of
 // the same kernel.  The test hook and the large-|beta| variant are always run-time geometry.
 template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE = false>
 int launch_sweep(xy_ctx* c, const SweepParams& P) {
@@ -198,6 +205,7 @@ int launch_sweep(xy_ctx* c, const SweepParams& P) {
         if (P.W4 == 20 && P.TY == 16) return launch_sweep_impl<MODE, false, FUSED, false, 20, 16>(c, P);
         if (P.W4 == 16 && P.TY == 16) return launch_sweep_impl<MODE, false, FUSED, false, 16, 16>(c, P);
         if (P.W4 == 12 && P.TY == 16) return launch_sweep_impl<MODE, false, FUSED, false, 12, 16>(c, P);
+        if (P.W4 == 10 && P.TY == 16) return launch_sweep_impl<MODE, false, FUSED, false, 10, 16>(c, P);
         if (P.W4 == 8 && P.TY == 32) return launch_sweep_impl<MODE, false, FUSED, false, 8, 32>(c, P);
         if (P.W4 == 4 && P.TY == 32) return launch_sweep_impl<MODE, false, FUSED, false, 4, 32>(c, P);
     }
@@ -486,8 +494,15 @@ xy_ctx* xy_create(int L, int R, const double* betas, uint64_t seed) {
             if (cost < best * 0.999) { best = cost; c->TZ_met = t; }
         }
     }
-    // L = 96 (a paper size): 16 rows x 12 float4 = 6 whole warps with uniform x parity -> the compile-time variant
-    if (L == 96 && tiles_ok(L, 16, c->TZ)) c->TY = 16;
+    // L = 96 and L = 80 (paper sizes): 16 rows x 12 (10) float4 = 6 (5) whole warps -> the compile-time variants
+    // (L = 96 with warps of uniform x parity; L = 80: 0.1587 -> 0.1526 ms per step at R = 34 against 20 rows, run-time geometry)
+    if ((L == 96 || L == 80) && tiles_ok(L, 16, c->TZ)) {
+        c->TY = 16;
+        default_tiles_z(L, R, 16, c->TZ);
+        // measured at the paper's R = 34 (bench.py --family): L = 80: TZ 16 0.1468 ms per step against 0.1526 (20), 0.1786 (40);
+        // L = 96: TZ 24 0.2405 against 0.2594 (32) -- three blocks of these small tiles fit an SM, which the model does not know
+        if (R >= 24 && R <= 48) c->TZ = L == 80 ? 16 : 24;
+    }
     return c;
 }
 

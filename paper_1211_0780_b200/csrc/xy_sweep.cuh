@@ -130,8 +130,8 @@ __host__ __device__ inline size_t sweep_smem_bytes(int L, int TY) {
 }
 
 // W4C, TYC: L/8 and the tile rows as compile-time constants (every shared-memory pitch becomes an
-// immediate, and TYC*W4C/2 is a multiple of 32 so that the x parity of a warp's sites is uniform),
-// or 0, 0 = read the geometry from P, any tile.
+// immediate; where TYC*W4C/2 is a multiple of 32 the warps are mapped to rows of one parity, so that the
+// x parity of a warp's sites is uniform), or 0, 0 = read the geometry from P, any tile.
 // EXACT_INLINE (Metropolis only): re-evaluate close decisions in fp64 on the spot (function call in
 // the loop: slow; chosen by the launcher when |beta| is so large that most decisions are "close").
 // Otherwise close decisions are appended to a global queue and settled by met_fixup_kernel, which
@@ -143,9 +143,9 @@ __host__ __device__ inline size_t sweep_smem_bytes(int L, int TY) {
 #define XY_MET_EARLY_DRAW 1
 #endif
 template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE, int W4C, int TYC>
-__global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 384, (W4C * TYC > 352) ? 1 : XY_SWEEP_MIN_BLOCKS) sweep_kernel(const SweepParams P) {
+__global__ void __launch_bounds__(W4C ? (W4C * TYC + 31) / 32 * 32 + 32 : 384, (W4C * TYC > 352) ? 1 : XY_SWEEP_MIN_BLOCKS) sweep_kernel(const SweepParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    constexpr bool UNI = W4C != 0;
+    constexpr bool UNI = W4C != 0 && (W4C * TYC / 2) % 32 == 0;   // whole warps per row parity (L = 80: compile-time geometry only)
     const int L = P.L;
     const int W4 = W4C ? W4C : P.W4;
     const int W = 4 * W4;
@@ -258,7 +258,7 @@ __global__ void __launch_bounds__(W4C ? W4C * TYC + 32 : 384, (W4C * TYC > 352) 
         // ---- compute warps.  This thread's own item: row ty of the tile, float4 column q; idle threads
         //      (compute threads rounded up to a warp) shadow item 0 and store nothing.  UNI: warps
         //      [0, n/2) take the even rows, the rest the odd rows, so the x parity is uniform over a warp
-        active = UNI || tid < P.nItems;
+        active = (W4C != 0 && (W4C * TYC) % 32 == 0) || tid < P.nItems;
         const int item = active ? tid : 0;
         int ty, q;
         if (UNI) {
