@@ -809,6 +809,30 @@ def test_slot_chunk_schedule_equals_default(xy_mod, L, R, chunk, n_or):
         assert np.array_equal(o[4], ref[4]) and np.array_equal(o[5], ref[5])
 
 
+@pytest.mark.parametrize("L,R", [(16, 6), (64, 3)])
+def test_checkpoint_resume_is_bitwise(xy_mod, L, R):
+    """SURVEY section 5 (checkpoint / resume): state, permutation and counters read through the C ABI and restored into a
+    NEW context continue the trajectory bit for bit -- the chain is a deterministic function of (seed, betas, state,
+    labels, counters).  L = 16 runs the resident kernel, L = 64 the per-pass kernels under graph replay."""
+    betas = inputs.beta_ladder(0.45, 0.46, R)
+    ref = xy_mod.XY(L, R, betas, SEED)
+    ref.init_random()
+    ref.mcs(20)
+    a = xy_mod.XY(L, R, betas, SEED)
+    a.init_random()
+    a.mcs(9)
+    state, perm, counters = a.get_state(), a.get_perm(), a.get_counters()
+    a.close()
+    b = xy_mod.XY(L, R, betas, SEED)
+    b.set_state(state); b.set_perm(perm); b.set_counters(counters)
+    b.mcs(11)
+    assert list(b.get_counters()) == list(ref.get_counters())
+    assert np.array_equal(b.get_perm(), ref.get_perm())
+    assert np.array_equal(b.get_state().view(np.uint32), ref.get_state().view(np.uint32))
+    assert np.array_equal(b.get_beta_of_slot(), ref.get_beta_of_slot())
+    assert np.array_equal(b.measure(), ref.measure())
+
+
 def test_mcs_with_several_overrelaxation_sweeps(xy_mod):
     """XY_OPT_OR_PER_MCS: xy_mcs must equal the same calls made one by one, bit for bit, and its
     series rows must be the observables of the state the last over-relaxation sweep left behind."""
