@@ -219,6 +219,56 @@ int xy_get_kernel_times(xy_ctx* ctx, double* ms, uint64_t* launches);
 int xy_synchronize(xy_ctx* ctx);
 const char* xy_last_error(void);
 
+/* ---- the observable reduction for callers that cannot allocate device memory ----------------- */
+
+/* Capacity of the library's built-in scratch area used by xy_measure_static, in bytes. */
+#define XY_STATIC_SCRATCH_BYTES (1u << 20)
+
+/* E, Mx, My, |M|^2, |M|^4 [P:52-56 Eqs. 4-5] of R spin configurations, WITHOUT a context, a workspace or any
+ * allocation: the call neither runs cudaMalloc / cudaFree nor any library routine that allocates.
+ *
+ * Who needs this.  Every other entry point works on an xy_ctx whose workspace (xy_workspace_bytes: 50 MB at
+ * L = 160 x 64) somebody has to allocate -- the caller before xy_attach, or xy_attach itself with cudaMalloc.
+ * Some code that holds a spin state can do neither: an analysis or monitoring hook that is only lent the state
+ * buffer by a simulation which has already given the rest of the GPU to its own memory pool (a raw cudaMalloc
+ * then fails, or is forbidden by the host program's rules); a service loop that must not stall, where
+ * cudaMalloc / cudaFree are unacceptable because they synchronise the whole device; a process whose memory
+ * budget is fixed at start-up.  For them the reduction's scratch (the per-tile partial sums between its two
+ * kernels) lives in an array compiled into the library, XY_STATIC_SCRATCH_BYTES = 1 MiB of device memory that
+ * every GPU holds from the moment it loads this library's code until the process exits.
+ *
+ * d_state:  DEVICE pointer, the colour-split state exactly as the library keeps it in the d_state buffer of
+ *           xy_attach (top of this file: black half-lattices of all R slots, then the white ones; R*N floats,
+ *           angles in [0, 2 pi]), 16-byte aligned, on the CURRENT device.  Read only.
+ * d_out:    DEVICE pointer, R*5 doubles, written as out[slot][5] -- indexed by SLOT, not by rank: there is no
+ *           context here and therefore no permutation (xy_get_perm maps ranks to slots).
+ * cuda_stream: a cudaStream_t on the current device (NULL = the default stream).  The two kernels are
+ *           enqueued there; the call does not synchronise and d_out is valid once the stream has reached
+ *           the end of this call's work.
+ *
+ * Same kernels and arithmetic as xy_measure (fp32 site terms, fp64 fixed-order sums, deterministic); the
+ * tiles are the library's defaults for (L, R) and always the run-time-geometry kernel, so against xy_measure
+ * on a context with other tiles the sums differ by rounding only (well inside 1e-6 * 3N).
+ *
+ * Limit.  The scratch need is 24 bytes x R x (thread-block tiles per replica).  All five BASELINE configs and
+ * the paper's families need under 64 KiB; a shape that needs more than XY_STATIC_SCRATCH_BYTES (e.g. L = 8
+ * with R > 43690) is refused with XY_ERR_INVALID_ARG and a message that names need and capacity; nothing is
+ * enqueued.  Use xy_measure on a context for those.
+ *
+ * First call on a device.  The first call made while a given device is current looks up the device address
+ * of the built-in array and raises the kernel's shared-memory limit, once per device.  That set-up is not
+ * stream work: make this first call at start-up, before any stream capture is begun on that device.
+ *
+ * Sharing.  There is ONE scratch array per device and every call uses it, whatever the stream or host
+ * thread.  It keeps whatever the previous call left there; that is harmless because each call's first kernel
+ * overwrites every entry its second kernel reads (nothing has to start at zero, nothing is cleared).  But two
+ * calls whose kernels can overlap on the GPU -- different streams without an event between them, or two host
+ * threads -- race on it and both get garbage: keep calls on one stream, or order them with events.
+ *
+ * Errors: XY_ERR_INVALID_ARG (shape, size beyond the scratch, NULL / misaligned / non-device / wrong-device
+ * pointer), XY_ERR_NO_DEVICE (no sm_100 device current), XY_ERR_CUDA. */
+int xy_measure_static(const float* d_state, int L, int R, double* d_out, void* cuda_stream);
+
 /* ---- test hooks (stated-error measurements; not part of the Monte Carlo step) ---------------- */
 
 /* With XY_OPT_TRACE = 1: the fast-path acceptance probability min(p_fast, FLT_MAX) of every site

@@ -11,7 +11,7 @@ __all__ = ["inputs", "XY", "load_library", "build_library"]
 
 
 def __getattr__(name):
-    if name in ("XY", "load_library", "XYError", "debug_sincos", "debug_sincos64", "debug_atan2", "debug_philox"):
+    if name in ("XY", "load_library", "XYError", "measure_static", "debug_sincos", "debug_sincos64", "debug_atan2", "debug_philox"):
         from . import binding
         return getattr(binding, name)
     if name == "build_library":

@@ -53,6 +53,7 @@ SIGNATURES = {
     "xy_get_kernel_times": (_i, [_vp, _pd, _pu64]),
     "xy_synchronize": (_i, [_vp]),
     "xy_last_error": (C.c_char_p, []),
+    "xy_measure_static": (_i, [_vp, _i, _i, _vp, _vp]),
     "xy_debug_get_trace": (_i, [_vp, _vp]),
     "xy_debug_sincos": (_i, [_vp, _vp, _vp, _sz, _vp]),
     "xy_debug_sincos64": (_i, [_vp, _vp, _vp, _sz, _vp]),
@@ -184,6 +185,11 @@ class XY:
         _check(_lib.xy_measure(self._h, out.ctypes.data), "xy_measure")
         return out
 
+    def measure_static(self, out=None):
+        """[R,5] CUDA fp64 tensor E, Mx, My, |M|^2, |M|^4 by SLOT of this object's spins through xy_measure_static, the
+        entry point that allocates nothing inside the library (see measure_static below).  Enqueued on self.stream."""
+        return measure_static(self._state, self.L, self.R, out=out, stream=self.stream)
+
     def pt_exchange(self):
         _check(_lib.xy_pt_exchange(self._h), "xy_pt_exchange")
 
@@ -276,6 +282,32 @@ class XY:
         a = np.empty((self.R, self.L, self.L, self.L), dtype=np.float32)
         _check(_lib.xy_debug_get_trace(self._h, a.ctypes.data), "xy_debug_get_trace")
         return a
+
+
+# ---- the reduction for callers that cannot allocate device memory ------------------------------
+def measure_static(state, L, R, out=None, stream=None):
+    """xy_measure_static of include/xy.h: observables by SLOT of a colour-split state the caller already holds.
+
+    The library allocates nothing in this call -- its scratch is a 1 MiB array compiled into libxy_b200.so -- which is
+    the point: it serves code that is lent a spin state but cannot get device memory of its own (everything already
+    given to another pool, no cudaMalloc allowed in a loop that must not stall, a fixed memory budget).  Pass `out`
+    (contiguous CUDA fp64 tensor of R*5 elements) to keep this wrapper allocation-free too; without it the wrapper
+    makes one small torch tensor for convenience.  state: CUDA tensor holding R*L^3 fp32 in the library's colour-split
+    layout (XY._state is one).  Asynchronous on `stream` (default: torch's current stream); calls share one scratch
+    array per device, so never let two of them overlap on the GPU.  Shapes whose partial sums exceed the array raise."""
+    torch = _torch()
+    lib = load_library()
+    n = int(R) * int(L) ** 3
+    if not state.is_cuda or state.numel() * state.element_size() < 4 * n or not state.is_contiguous():
+        raise XYError("measure_static: state must be a contiguous CUDA tensor of at least R*L^3 fp32")
+    if out is None:
+        out = torch.empty((int(R), NUM_OBS), dtype=torch.float64, device=state.device)
+    if not out.is_cuda or out.dtype != torch.float64 or not out.is_contiguous() or out.numel() != int(R) * NUM_OBS:
+        raise XYError("measure_static: out must be a contiguous CUDA fp64 tensor of R*5 elements")
+    with torch.cuda.device(state.device):
+        st = stream if stream is not None else torch.cuda.current_stream()
+        _check(lib.xy_measure_static(state.data_ptr(), int(L), int(R), out.data_ptr(), st.cuda_stream), "xy_measure_static")
+    return out
 
 
 # ---- test hooks: the kernels' device math on arrays -------------------------------------------

@@ -8,6 +8,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "xy_kernels.cuh"
@@ -1026,3 +1027,114 @@ int xy_debug_philox(const uint32_t* d_ctr, uint32_t key0, uint32_t key1, uint32_
 }
 
 }  // extern "C"
+
+// ---- xy_measure_static: the observable reduction with its scratch compiled into the library ------------------
+// For callers that may not allocate (include/xy.h says who and why).  The per-tile partial sums that travel from
+// the first kernel (sweep_kernel in MODE_MEASURE) to the second live in this file-scope array instead of a
+// workspace: 1 MiB that every device holds from the load of this module until the process exits.
+// NOTE for maintainers: in HOST code the name `xy_static_scratch` is only a handle for the runtime, not a device
+// address -- never pass it to a kernel.  static_setup() below asks the runtime for the real address once per
+// device (cudaGetSymbolAddress, with that device current) and the launch code passes THAT pointer.  Device code
+// (measure_finalize_static_kernel) may and does name the array directly.
+static __device__ __align__(256) unsigned char xy_static_scratch[XY_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+// Second stage of the static variant: one warp per SLOT sums that slot's tile partials out of the built-in array
+// in the same fixed order as finalize_rank (lane l takes tiles l, l+32, ..., then a shuffle tree); lane 0 writes
+// the five observables.  No permutation: the caller has no context, rows are by slot.
+__global__ void measure_finalize_static_kernel(int n_tiles, int R, double* __restrict__ out_slot) {
+    const int slot = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (slot >= R) return;
+    const double* __restrict__ partials = reinterpret_cast<const double*>(xy_static_scratch);
+    double v[3] = { 0.0, 0.0, 0.0 };
+    for (int t = lane; t < n_tiles; t += 32)
+        for (int c = 0; c < 3; ++c) v[c] += partials[((size_t)slot * n_tiles + t) * 3 + c];
+    for (int c = 0; c < 3; ++c)
+        for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
+    if (lane == 0) {
+        const double m2 = v[1] * v[1] + v[2] * v[2];
+        out_slot[5 * slot + 0] = v[0]; out_slot[5 * slot + 1] = v[1]; out_slot[5 * slot + 2] = v[2];
+        out_slot[5 * slot + 3] = m2;   out_slot[5 * slot + 4] = m2 * m2;
+    }
+}
+
+// Per-device set-up of the static variant, done by the first xy_measure_static call that finds the device current:
+// the device address of the array on THIS device and the first kernel's dynamic-shared-memory opt-in.  Neither
+// allocates; neither is stream work (hence "first call before any stream capture" in xy.h).
+struct StaticDevice { bool ready = false; double* scratch = nullptr; };
+StaticDevice g_static_dev[kMaxDevices];
+std::mutex g_static_mutex;
+
+int static_setup(int dev, double** scratch) {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice& s = g_static_dev[dev];
+    if (!s.ready) {
+        int major = 0;
+        CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        if (major < 10) return fail(XY_ERR_NO_DEVICE, "xy_measure_static: device %d is sm_%dx; built for sm_100a only", dev, major);
+        void* p = nullptr;
+        CK(cudaGetSymbolAddress(&p, xy_static_scratch));       // valid for the device that is current now, i.e. `dev`
+        if (!p) return fail(XY_ERR_CUDA, "xy_measure_static: cudaGetSymbolAddress returned a null address");
+        CK(cudaFuncSetAttribute(sweep_kernel<MODE_MEASURE, false, false, false, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        s.scratch = static_cast<double*>(p);
+        s.ready = true;
+    }
+    *scratch = s.scratch;
+    return XY_OK;
+}
+
+}  // namespace
+
+extern "C" int xy_measure_static(const float* d_state, int L, int R, double* d_out, void* cuda_stream) {
+    if (!shape_ok(L, R)) return fail(XY_ERR_INVALID_ARG, "xy_measure_static: need L %% 8 == 0, 8 <= L <= 1024, 1 <= R <= 65535 (got L=%d R=%d)", L, R);
+    int TY = 0, TZ = 0;
+    default_tiles(L, R, TY, TZ);
+    if (!tiles_ok(L, TY, TZ)) return fail(XY_ERR_INVALID_ARG, "xy_measure_static: no valid tile for L=%d (TY=%d TZ=%d)", L, TY, TZ);
+    // the whole size check comes before anything touches the device: a shape beyond the built-in array is refused
+    const size_t n_tiles = (size_t)(L / TY) * (size_t)(L / TZ);
+    const size_t need = (size_t)R * n_tiles * 3 * sizeof(double);
+    if (need > (size_t)XY_STATIC_SCRATCH_BYTES)
+        return fail(XY_ERR_INVALID_ARG,
+                    "xy_measure_static: L=%d R=%d needs %zu bytes of scratch (24 x %d replicas x %zu tiles) but the built-in array holds %zu; "
+                    "use xy_measure on a context for this size", L, R, need, R, n_tiles, (size_t)XY_STATIC_SCRATCH_BYTES);
+    if (!d_state || !d_out) return fail(XY_ERR_INVALID_ARG, "xy_measure_static: NULL pointer");
+    if (((uintptr_t)d_state & 15u) || ((uintptr_t)d_out & 7u)) return fail(XY_ERR_INVALID_ARG, "xy_measure_static: d_state must be 16-byte and d_out 8-byte aligned");
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) {
+        cudaGetLastError();
+        return fail(XY_ERR_NO_DEVICE, "xy_measure_static: no CUDA device; this library has no CPU fallback");
+    }
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return fail(XY_ERR_NO_DEVICE, "xy_measure_static: device index %d out of range", dev);
+    for (const void* p : { (const void*)d_state, (const void*)d_out }) {      // both must be device memory of the current device
+        cudaPointerAttributes pa;
+        if (cudaPointerGetAttributes(&pa, p) != cudaSuccess) { cudaGetLastError(); return fail(XY_ERR_INVALID_ARG, "xy_measure_static: not a CUDA pointer"); }
+        if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) return fail(XY_ERR_INVALID_ARG, "xy_measure_static: d_state and d_out must be device memory");
+        if (pa.type == cudaMemoryTypeDevice && pa.device != dev)
+            return fail(XY_ERR_INVALID_ARG, "xy_measure_static: a buffer lives on device %d but the current device is %d", pa.device, dev);
+    }
+    double* scratch = nullptr;
+    if (const int rc = static_setup(dev, &scratch)) return rc;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+
+    const size_t half_n = (size_t)L * L * L / 2;
+    SweepParams P;
+    memset(&P, 0, sizeof(P));
+    P.own = const_cast<float*>(d_state) + (size_t)R * half_n;      // own = white (MODE_MEASURE stores nothing to it), staged = black
+    P.other = d_state;
+    P.L = L; P.W = L / 2; P.W4 = L / 8;
+    P.TY = TY; P.TZ = TZ; P.nTY = L / TY; P.nTZ = L / TZ;
+    P.colour = 1;
+    P.slot0 = 0; P.n_slots = R;
+    P.nItems = TY * P.W4;
+    P.half_n = (unsigned int)half_n;
+    P.partials = scratch;                                          // the device address from cudaGetSymbolAddress, never the symbol
+    const int threads = (P.nItems + 31) / 32 * 32 + 32;            // compute warps + the auxiliary warp
+    sweep_kernel<MODE_MEASURE, false, false, false, 0, 0><<<dim3(P.nTY * P.nTZ, R), threads, sweep_smem_bytes(L, TY), stream>>>(P);
+    CK(cudaGetLastError());
+    measure_finalize_static_kernel<<<(R + 3) / 4, 128, 0, stream>>>((int)n_tiles, R, d_out);
+    CK(cudaGetLastError());
+    return XY_OK;
+}
