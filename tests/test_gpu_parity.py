@@ -669,7 +669,11 @@ def test_set_state_reduces_out_of_range_angles(xy_mod, oracle_mod):
 
 # ---- f2 stage A: the resident kernel (whole steps of a small lattice in one persistent launch) ------------------
 @pytest.mark.parametrize("L,R,n_or", [(8, 8, 1), (8, 3, 1), (8, 20, 2), (8, 64, 1), (16, 4, 1), (16, 5, 0), (24, 2, 1), (32, 3, 1),
-                                      (32, 16, 1), (40, 2, 1), (48, 2, 2)])
+                                      (32, 16, 1), (40, 2, 1), (48, 2, 2),
+                                      # several slots per thread block (R > 132 blocks' worth): the slot split of the
+                                      # threads, a partially filled last block (R = 133: 66 full blocks + one slot),
+                                      # the tag exchange between many one-block "clusters"
+                                      (8, 133, 1), (8, 200, 1), (8, 512, 1), (16, 200, 1)])
 def test_resident_kernel_equals_per_pass_kernels(xy_mod, L, R, n_or):
     """XY_OPT_RESIDENT: n whole steps in one launch with the spins resident in shared
     memory must leave BITWISE the states, labels, counters and Metropolis / exchange acceptance counts of the
@@ -684,6 +688,10 @@ def test_resident_kernel_equals_per_pass_kernels(xy_mod, L, R, n_or):
         xy = xy_mod.XY(L, R, betas, SEED)
         xy.set_option(xy_mod.XY_OPT_RESIDENT, resident)
         xy.set_option(xy_mod.XY_OPT_OR_PER_MCS, n_or)
+        if resident:
+            plan = xy.get_resident_plan()
+            assert plan["resident"] == 1, plan
+            assert (plan["slots_per_block"] > 1) == (R > 132), plan
         xy.init_random()
         s1 = torch.zeros(6, R, 5, dtype=torch.float64, device="cuda")
         s2 = torch.zeros(5, R, 5, dtype=torch.float64, device="cuda")
@@ -709,40 +717,111 @@ def test_resident_kernel_equals_per_pass_kernels(xy_mod, L, R, n_or):
     assert np.array_equal(a[9].view(np.uint32), b[9].view(np.uint32)) and np.array_equal(a[10], b[10])
 
 
-def test_resident_kernel_lockstep_against_oracle(xy_mod, oracle_mod):
-    """The resident kernel against the ORACLE directly (not only against the other kernels): one xy_mcs(1) from a
-    shared state is one oracle MCS -- Metropolis decisions read off the state pass by pass are not available here
-    (the four passes run in one launch), so the check is the composed one: after Metropolis + over-relaxation the
-    angles agree within the P2 clause wherever the two Metropolis sweeps took the same decisions, which the fp64
-    settlement guarantees; observables and the exchange follow P3 / P4."""
-    for L, R in ((8, 8), (16, 3), (32, 4)):
-        betas = inputs.beta_ladder(0.45, 0.458, R)
-        xy, ora = make(xy_mod, oracle_mod, L, R, betas=betas)
-        assert xy.get_option(xy_mod.XY_OPT_RESIDENT) == 1
-        xy.init_random(); xy.mcs(4)
-        for t in (4, 5):
-            S, perm = xy.get_state(), xy.get_perm()
-            ora.set_state(S); ora.set_perm(perm); ora.set_counters([t, t, t])
-            import torch
-            row = torch.zeros(1, R, 5, dtype=torch.float64, device="cuda")
-            xy.mcs(1, row)
-            ora.metropolis_sweep()
-            ora.overrelax_sweep()
-            O = ora.get_state()
-            G = xy.get_state()
-            # where a Metropolis decision differed the site would be off by O(1): none may
-            d = H.angle_diff(G, O)
-            assert d.max() <= 5e-3, f"a decision differs (max angle difference {d.max():.3e})"
-            assert (d > P.TOL_ANGLE).mean() <= 2e-4
-            P.check_observables(xy.measure(), ora_obs_of(G, ora, xy.get_perm()), L ** 3)     # by rank AFTER the exchange
-            # the exchange decisions were taken on the GPU's energies; replay them in the oracle from the same energies
-            tr = ora.enable_trace(pt=True)
-            ora.set_state(G); ora.set_perm(perm); ora.set_counters([t + 1, t + 1, t])
-            ora.pt_exchange()
-            P.check_pt(xy.get_perm(), ora.get_perm(), tr["pt_p"], tr["pt_u"])
-            ora.enable_trace()
-            assert np.array_equal(xy.get_counters(), [t + 1, t + 1, t + 1])
-            P.check_observables(row.cpu().numpy()[0], ora_obs_of(G, ora, perm), L ** 3)
+def xy_mcs_lockstep(xy_mod, xy, ora, S, perm, t):
+    """ONE xy_mcs(1) call against the oracle, stage by stage (P1-P4 directly, for the paths that run a whole step
+    without handing the intermediate states back: the resident kernel, the slot-chunk schedule).
+
+    (a) P1.  With XY_OPT_OR_PER_MCS = 0 the call is Metropolis sweep + reduction + exchange, so the state it leaves is
+        the Metropolis result M: every site bitwise old-or-proposal, decisions against the oracle's trace, pass by
+        pass (the oracle's white pass starts from the GPU's own black result), exactly like metropolis_lockstep.
+    (b) P2.  The same call from the same state and counters with one over-relaxation sweep leaves G; the Metropolis
+        part is deterministic, so the over-relaxation went from M to G: the oracle's two passes from M with its |h|
+        trace, under the conditioning clause of check_overrelax.
+    (c) P3 / P4.  The series row of that call (by rank, before the exchange) against the oracle's observables of G,
+        and the exchange replayed in the oracle from the same energies."""
+    import torch
+    L, R = xy.L, xy.R
+    col = H.colour_mask(L)
+    prop, _ = H.predicted_proposals(L, R, t, SEED)
+    stats = {}
+    xy.set_option(xy_mod.XY_OPT_OR_PER_MCS, 0)
+    xy.set_state(S); xy.set_perm(perm); xy.set_counters([t, t, t])
+    xy.mcs(1)
+    M = xy.get_state()
+    assert np.array_equal(xy.get_counters(), [t + 1, t, t + 1])
+    ora.set_active_slots(None); ora.set_perm(perm); ora.set_counters([t, t, t])
+    start = S
+    for c in (0, 1):
+        sel = np.broadcast_to(col == c, S.shape)
+        ora.set_state(start)
+        tr = ora.enable_trace(met=True)
+        ora.metropolis_pass(c)
+        stats[f"met{c}"] = P.check_metropolis(start, M, ora.get_state(), prop, tr["met_p"], tr["met_u"], sel)
+        start = np.where(col[None] == 0, M, S)
+    ora.enable_trace()
+    xy.set_option(xy_mod.XY_OPT_OR_PER_MCS, 1)
+    xy.set_state(S); xy.set_perm(perm); xy.set_counters([t, t, t])
+    row = torch.zeros(1, R, 5, dtype=torch.float64, device="cuda")
+    xy.mcs(1, row)
+    G = xy.get_state()
+    assert np.array_equal(xy.get_counters(), [t + 1, t + 1, t + 1])
+    start = M
+    for c in (0, 1):
+        sel = np.broadcast_to(col == c, S.shape)
+        ora.set_state(start)
+        tr = ora.enable_trace(overrelax=True)
+        ora.overrelax_pass(c)
+        stats[f"or{c}"] = P.check_overrelax(G, ora.get_state(), tr["or_h"], sel)
+        start = np.where(col[None] == 0, G, M)
+    ora.enable_trace()
+    stats["obs"] = P.check_observables(row.cpu().numpy()[0], ora_obs_of(G, ora, perm), L ** 3)
+    tr = ora.enable_trace(pt=True)
+    ora.set_state(G); ora.set_perm(perm); ora.set_counters([t + 1, t + 1, t])
+    ora.pt_exchange()
+    P.check_pt(xy.get_perm(), ora.get_perm(), tr["pt_p"], tr["pt_u"])
+    ora.enable_trace()
+    P.check_observables(xy.measure(), ora_obs_of(G, ora, xy.get_perm()), L ** 3)      # by rank AFTER the exchange
+    return stats, G
+
+
+# (L, R, warm-up MCS, config index or None).  Every code path of the resident kernel: configs 1 and 2 as they are
+# benchmarked; several slots per block (R > 132), with a partially filled last block (R = 133); one block per slot and
+# clusters of 2, 4, 8 blocks per slot (the planner takes the largest co-resident cluster, so R decides); every lattice
+# size that has a kernel; a random start (warm = 0) and an equilibrated state (50 steps).
+RESIDENT_LOCKSTEP = [(8, 8, 0, 0), (8, 8, 50, 0), (8, 133, 0, None), (8, 200, 50, None),          # one block per slot; two slots per block
+                     (16, 3, 50, None), (16, 100, 0, None), (16, 140, 50, None),             # 8 blocks per slot; 1; two slots per block
+                     (24, 5, 0, None), (24, 30, 50, None), (24, 60, 0, None), (24, 100, 0, None),   # 8, 4, 2, 1 blocks per slot
+                     (32, 16, 50, 1), (32, 16, 0, 1), (32, 3, 0, None), (32, 36, 0, None),  # 4 (config 2), 8, 2 blocks per slot
+                     (40, 2, 0, None), (48, 2, 50, None)]
+
+
+@pytest.mark.parametrize("L,R,warm,cfg", RESIDENT_LOCKSTEP)
+def test_resident_kernel_lockstep_P1_P2_against_oracle(xy_mod, oracle_mod, L, R, warm, cfg):
+    """The default xy_mcs path of configs 1-2 (L <= 48: resident_mcs_kernel) against the ORACLE with the same bars as
+    the per-pass kernels: P1 decision by decision, P2 with the conditioning clause, P3, P4 (xy_mcs_lockstep)."""
+    betas = inputs.betas_of(inputs.CONFIGS[cfg]) if cfg is not None else inputs.beta_ladder(0.45, 0.458, R)
+    xy, ora = make(xy_mod, oracle_mod, L, R, betas=betas)
+    plan = xy.get_resident_plan()
+    assert xy.get_option(xy_mod.XY_OPT_RESIDENT) == 1 and plan["resident"] == 1, plan
+    assert (plan["slots_per_block"] > 1) == (R > 132), plan
+    xy.init_random()
+    if warm:
+        xy.mcs(warm)
+    S, perm = xy.get_state(), xy.get_perm()
+    for t in (warm, warm + 1):
+        stats, S = xy_mcs_lockstep(xy_mod, xy, ora, S, perm, t)
+        perm = xy.get_perm()
+        print(L, R, "t", t, "plan", plan, stats)
+    # two resident launches per lock-step (plus the layout conversions, the standalone rank gather of xy_measure ...):
+    # no Metropolis / over-relaxation colour-pass kernel ran
+    xy.set_option(xy_mod.XY_OPT_PROFILE, 1); xy.get_kernel_times()
+    xy.mcs(1)
+    kt = xy.get_kernel_times()
+    assert kt["resident"][1] == 1 and kt["metropolis"][1] == 0 and kt["overrelax"][1] == 0, kt
+
+
+def test_slot_chunk_step_lockstep_against_oracle(xy_mod, oracle_mod):
+    """XY_OPT_SLOT_CHUNK against the ORACLE (not only against the default schedule): one xy_mcs(1) at L = 64 with the
+    passes of 2 of 3 slots back to back (a ragged last chunk), P1-P4 stage by stage, from an equilibrated state."""
+    L, R = 64, 3
+    xy, ora = make(xy_mod, oracle_mod, L, R, betas=inputs.beta_ladder(0.4530, 0.4555, R))
+    xy.set_option(xy_mod.XY_OPT_SLOT_CHUNK, 2)
+    xy.init_random(); xy.mcs(20)
+    S, perm = xy.get_state(), xy.get_perm()
+    for t in (20, 21):
+        stats, S = xy_mcs_lockstep(xy_mod, xy, ora, S, perm, t)
+        perm = xy.get_perm()
+        print(L, R, "chunk 2, t", t, stats)
 
 
 def ora_obs_of(state, ora, perm):
