@@ -65,8 +65,17 @@ enum {
                               step on (counters live on the device); 0: every kernel is launched eagerly  */
     XY_OPT_RESIDENT = 9,   /* 1 (default): for small lattices (L = 8 ... 48, R <= 512, everything co-resident) xy_mcs
                               runs all its steps in ONE persistent launch with the spins resident in shared
-                              memory (same results: states, labels and counters bitwise, observables
-                              within the reduction's rounding); 0: always the per-pass kernels                 */
+                              memory.  Same site arithmetic and Philox keying as the per-pass kernels:
+                              the spins after a call are bitwise theirs, the observables agree within the reduction's
+                              rounding (their fp32 terms are grouped differently).  The exchange compares log(u) < x
+                              where the per-pass kernels compare u < exp(x), on energies that differ by that rounding:
+                              a decision within about 1e-8 of its threshold can fall the other way (inside the 1e-6
+                              window of P4), and from such a step on the two trajectories part -- both are valid, only
+                              bitwise equality between the two paths is lost (never seen in the tests' runs).
+                              While this path is taken, XY_OPT_TILE_Y / TILE_Z / GENERIC_KERNEL / FUSED_MEASURE /
+                              CUDA_GRAPH / SLOT_CHUNK do not apply to xy_mcs (they still govern the sweep-by-sweep
+                              calls); XY_OPT_TRACE = 1 forces the per-pass kernels (xy_get_resident_plan says which
+                              path xy_mcs takes).  0: always the per-pass kernels                                */
     XY_OPT_SLOT_CHUNK = 10 /* K > 0: xy_mcs runs the four colour passes of K slots at a time back to back (launches
                               over slots [0,K), [K,2K), ...) so that a chunk's spins stay in the 126 MB L2 between
                               its passes: 8 instead of 24 B of HBM traffic per site and step (SURVEY 8(f) f2 for
@@ -96,8 +105,8 @@ enum {
  * betas); the reason is in xy_last_error().  [north_star: xy_create(L, R, betas, seed)] */
 xy_ctx* xy_create(int L, int R, const double* betas, uint64_t seed);
 
-/* Frees the context and whatever it allocated itself; attached caller-owned buffers and the
- * stream are not touched.  NULL is allowed. */
+/* Frees the context and whatever it allocated itself (on the context's device, whichever device is current);
+ * attached caller-owned buffers and the stream are not touched.  NULL is allowed. */
 void xy_destroy(xy_ctx* ctx);
 
 /* Bytes of device memory a context of this shape needs: the colour-split state (R*N floats)
@@ -108,7 +117,8 @@ size_t xy_workspace_bytes(int L, int R);
 
 /* Binds device memory and a stream.  d_state / d_workspace: DEVICE pointers, 256-byte aligned,
  * of at least xy_state_bytes / xy_workspace_bytes, on the CURRENT device, owned by the caller
- * (PyTorch) and required to outlive the context.  The context is bound to the device that is
+ * (PyTorch) and required to outlive the context.  A caller's stream must belong to the current device too
+ * (XY_ERR_INVALID_ARG otherwise).  The context is bound to the device that is
  * current at this call: every later entry point switches to it for its own duration and restores
  * the caller's current device.  Either buffer may be NULL, in which case the library cudaMallocs and owns it.
  * cuda_stream: a cudaStream_t; NULL = the library creates a blocking stream of its own, which is
@@ -206,7 +216,7 @@ int xy_get_exact_path_count(xy_ctx* ctx, uint64_t* n);
 int xy_set_option(xy_ctx* ctx, int option, int value);
 int xy_get_option(xy_ctx* ctx, int option, int* value);
 /* How xy_mcs will run on this context (XY_OPT_RESIDENT): out[0] = 1 if all steps of a call run in one persistent
- * launch with the spins resident in shared memory, else 0 (per-pass kernels); out[1] = slots per thread block,
+ * launch with the spins resident in shared memory, else 0 (per-pass kernels: no plan fits, XY_OPT_RESIDENT = 0 or XY_OPT_TRACE = 1); out[1] = slots per thread block,
  * out[2] = thread blocks (cluster size) per slot, out[3] = threads per block, out[4] = blocks, out[5] = dynamic
  * shared memory per block in bytes.  The plan needs the device: call after xy_attach. */
 int xy_get_resident_plan(xy_ctx* ctx, int out[6]);

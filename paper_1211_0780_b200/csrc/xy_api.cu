@@ -372,7 +372,8 @@ int resident_launch(xy_ctx* c, const ResidentPlan& pl, const ResidentParams& P, 
     // the CTAs wait on one another once per step: co-residency is guaranteed by a cooperative launch
     at[na].id = cudaLaunchAttributeCooperative; at[na].val.cooperative = 1; ++na;
     cfg.numAttrs = na;
-    CK(cudaMemsetAsync(c->ws_ptr<unsigned int>(c->ws.res_sync), 0, 8, c->stream));
+    // res_sync[1], the kernel's "aborted" flag, is zeroed by xy_attach only: like the close-decision overflow flag it stays
+    // set until the context is attached again, so a second xy_mcs enqueued before any synchronising call cannot wipe it
     if (pl.grid > 1) CK(cudaMemsetAsync(c->ws_ptr<char>(c->ws.res_xchg), 0, (size_t)2 * c->R * kResMaxC * 6 * 8, c->stream));   // step tags start at 1
     {
         LaunchSpan span(c, XY_K_RESIDENT);
@@ -509,6 +510,8 @@ xy_ctx* xy_create(int L, int R, const double* betas, uint64_t seed) {
 
 void xy_destroy(xy_ctx* c) {
     if (!c) return;
+    DeviceScope scope;                             // free buffers, stream, events and graph on the device they belong to
+    if (c->device >= 0) scope.enter(c->device);
     if (c->own_state && c->d_state) cudaFree(c->d_state);
     if (c->own_ws && c->d_ws) cudaFree(c->d_ws);
     if (c->d_trace) cudaFree(c->d_trace);
@@ -547,6 +550,18 @@ int xy_attach(xy_ctx* c, void* d_state, void* d_workspace, void* cuda_stream) {
             return fail(XY_ERR_INVALID_ARG, "xy_attach: buffer lives on device %d but the current device is %d", pa.device, dev);
     }
     c->stream = (cudaStream_t)cuda_stream;
+    if (c->stream) {                           // a caller's stream must belong to the device this context is bound to
+        int sdev = -1;
+        if (cudaStreamGetDevice(c->stream, &sdev) != cudaSuccess) {
+            cudaGetLastError();
+            c->stream = nullptr;
+            return fail(XY_ERR_INVALID_ARG, "xy_attach: cuda_stream is not a valid stream");
+        }
+        if (sdev != dev) {
+            c->stream = nullptr;
+            return fail(XY_ERR_INVALID_ARG, "xy_attach: the stream belongs to device %d but the current device is %d", sdev, dev);
+        }
+    }
     if (!c->stream) {                          // the legacy default stream cannot be captured into a graph: use a
         CK(cudaStreamCreate(&c->stream));      // BLOCKING stream of our own, which stays ordered with it
         c->own_stream = true;
@@ -813,7 +828,16 @@ int xy_mcs(xy_ctx* c, int n_mcs, double* d_series) {
     // XY_OPT_RESIDENT: small lattices run all n steps in ONE persistent launch with the spins resident in shared memory
     if (c->resident && !c->trace && n_mcs >= 1) {
         const ResidentPlan& pl = resident_plan(c);
-        if (pl.ok) return resident_mcs(c, pl, n_mcs, d_series);
+        if (pl.ok) {
+            // the kernel counts accepted proposals per thread in 32 bits over one launch: at most 2^24 steps per launch
+            // (a thread owns well under 2^7 sites), so xy_get_accept_counts stays exact for any n_mcs
+            constexpr int kMaxStepsPerLaunch = 1 << 24;
+            for (int done = 0; done < n_mcs; done += kMaxStepsPerLaunch) {
+                const int n = std::min(kMaxStepsPerLaunch, n_mcs - done);
+                if (const int rc = resident_mcs(c, pl, n, d_series ? d_series + (size_t)done * c->R * 5 : nullptr)) return rc;
+            }
+            return XY_OK;
+        }
     }
     int t = 0;
     // XY_OPT_CUDA_GRAPH: from the second step on, replay one captured graph per step (7 kernel nodes):
@@ -976,7 +1000,8 @@ int xy_get_resident_plan(xy_ctx* c, int out[6]) {
     ENTER(c);
     if (!out) return fail(XY_ERR_INVALID_ARG, "xy_get_resident_plan: NULL pointer");
     const ResidentPlan& pl = resident_plan(c);
-    out[0] = pl.ok && c->resident ? 1 : 0; out[1] = pl.G; out[2] = pl.C; out[3] = pl.threads; out[4] = pl.grid; out[5] = (int)pl.smem;
+    // XY_OPT_TRACE forces the per-pass kernels
+    out[0] = pl.ok && c->resident && !c->trace ? 1 : 0; out[1] = pl.G; out[2] = pl.C; out[3] = pl.threads; out[4] = pl.grid; out[5] = (int)pl.smem;
     return XY_OK;
 }
 

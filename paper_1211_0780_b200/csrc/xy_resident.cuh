@@ -526,12 +526,14 @@ __global__ void __launch_bounds__(resident_max_threads(L), 1) resident_mcs_kerne
             P.slot_at_rank[k] = sl; P.beta_of_slot[sl] = P.betas[k]; P.beta32_of_slot[sl] = (float)P.betas[k];
         }
     {
-        unsigned int a = live ? nacc : 0u, e = live ? nexact : 0u;
+        // widened BEFORE the warp sum: 32 lanes x up to 2^24 steps x the thread's sites does not fit 32 bits (the launcher
+        // caps a launch at 2^24 steps, which bounds the per-thread counters themselves)
+        unsigned long long a = live ? (unsigned long long)nacc : 0ull, e = live ? (unsigned long long)nexact : 0ull;
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, off); e += __shfl_xor_sync(0xffffffffu, e, off); }
         if ((tid & 31) == 0) {                                     // TPS is a multiple of 32: a warp belongs to one slot
-            if (a) atomicAdd(P.met_acc + slot, (unsigned long long)a);
-            if (e) atomicAdd(P.exact_count, (unsigned long long)e);
+            if (a) atomicAdd(P.met_acc + slot, a);
+            if (e) atomicAdd(P.exact_count, e);
         }
     }
     if (CLUSTER) cg::this_cluster().sync();                        // no CTA may leave while a neighbour could still write its halo

@@ -810,6 +810,30 @@ def test_resident_kernel_lockstep_P1_P2_against_oracle(xy_mod, oracle_mod, L, R,
     assert kt["resident"][1] == 1 and kt["metropolis"][1] == 0 and kt["overrelax"][1] == 0, kt
 
 
+def test_resident_plan_reports_the_path_xy_mcs_takes(xy_mod):
+    """xy_get_resident_plan()[0] is 1 exactly when xy_mcs will run the resident kernel: a plan exists, the option is
+    on and the Metropolis trace hook (which needs the per-pass kernels) is off; the kernel classes that actually ran
+    say the same."""
+    def classes_of_one_step(xy):
+        xy.set_option(xy_mod.XY_OPT_PROFILE, 1); xy.get_kernel_times()
+        xy.mcs(1)
+        kt = xy.get_kernel_times()
+        xy.set_option(xy_mod.XY_OPT_PROFILE, 0)
+        return kt["resident"][1], kt["metropolis"][1]
+    xy = xy_mod.XY(8, 8, inputs.beta_ladder(0.44, 0.47, 8), SEED)
+    xy.init_random()
+    assert xy.get_resident_plan()["resident"] == 1 and classes_of_one_step(xy) == (1, 0)
+    xy.set_option(xy_mod.XY_OPT_TRACE, 1)
+    assert xy.get_resident_plan()["resident"] == 0 and classes_of_one_step(xy) == (0, 2)
+    xy.set_option(xy_mod.XY_OPT_TRACE, 0)
+    assert xy.get_resident_plan()["resident"] == 1
+    xy.set_option(xy_mod.XY_OPT_RESIDENT, 0)
+    assert xy.get_resident_plan()["resident"] == 0 and classes_of_one_step(xy) == (0, 2)
+    big = xy_mod.XY(64, 2, inputs.beta_ladder(0.45, 0.46, 2), SEED)
+    big.init_random()
+    assert big.get_resident_plan()["resident"] == 0 and classes_of_one_step(big) == (0, 2)
+
+
 def test_slot_chunk_step_lockstep_against_oracle(xy_mod, oracle_mod):
     """XY_OPT_SLOT_CHUNK against the ORACLE (not only against the default schedule): one xy_mcs(1) at L = 64 with the
     passes of 2 of 3 slots back to back (a ragged last chunk), P1-P4 stage by stage, from an equilibrated state."""
