@@ -149,6 +149,43 @@ def run_reference(args, cfg):
     }))
 
 
+def time_other_workloads(binding, torch, skip_name, steps=20, warmup=5):
+    """Driver-timed numbers for the workloads the headline is NOT quoted on: BASELINE.json configs 1-4 and the paper's
+    own five families, `steps` steps of xy_mcs each after `warmup` (CUDA events, device-resident state,
+    the library's default path: the resident kernel for L <= 48, graph-replayed per-pass kernels above).  Configs 1-3
+    and the L = 64 family fit in the 126 MB L2 and are not flushed between steps (stated per entry): their numbers are
+    updates/ns, not an HBM roofline."""
+    work = [(c.name, c.L, c.R, inputs.betas_of(c), c.start, "linear in beta") for c in inputs.CONFIGS]
+    work += [(f.name, f.L, f.R, inputs.betas_of_family(f), f.start, "geometric in beta (PAPER.md:62 family)") for f in inputs.PAPER_FAMILIES]
+    out = []
+    for name, L, R, betas, start, ladder in work:
+        if name == skip_name:
+            continue
+        xy = binding.XY(L, R, betas, inputs.SEED)
+        xy.init_random() if start == "random" else xy.init_ordered(0.0)
+        xy.mcs(warmup)
+        torch.cuda.synchronize()
+        n0 = xy.get_launch_count()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        xy.mcs(steps)
+        b.record()
+        torch.cuda.synchronize()
+        xy.synchronize()                               # raises if a close-decision queue overflowed or a launch aborted
+        ms = a.elapsed_time(b) / steps
+        plan = xy.get_resident_plan()
+        state = 4 * L ** 3 * R
+        out.append({"workload": name, "L": L, "R": R, "ladder": ladder, "start": start, "steps": steps, "warmup": warmup,
+                    "ms_per_step": ms, "updates_per_ns": 2.0 * L ** 3 * R / (ms * 1e-3) * 1e-9,
+                    "path": ("resident kernel: %d block(s) per slot, %d slot(s) per block, %d blocks" % (plan["blocks_per_slot"], plan["slots_per_block"], plan["blocks"]))
+                            if plan["resident"] else "per-pass kernels, tiles %d x %d, graph replay" % (xy.get_option(binding.XY_OPT_TILE_Y), xy.get_option(binding.XY_OPT_TILE_Z)),
+                    "gpu_launches": xy.get_launch_count() - n0,
+                    "memory": "state %.1f MB: %s" % (state / 1e6, "L2-resident, no flush between steps" if state < 120e6 else "larger than L2 (HBM)"),
+                    "hbm_roofline_frac": (2.0 * L ** 3 * R * BYTES_PER_UPDATE / (ms * 1e-3) * 1e-9 / measured_peak_gbs()[0]) if state >= 120e6 else None})
+        xy.close()
+    return out
+
+
 def run_ours(args, cfg):
     import torch
     import torch.distributed as dist
@@ -265,7 +302,8 @@ def run_ours(args, cfg):
         "site_mcs_per_ns": units / 2 / (ms * 1e-3) * 1e-9,
         "hbm_roofline_frac_whole_mcs": units * BYTES_PER_UPDATE / (ms * 1e-3) * 1e-9 / peak,
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
-                     "frac": ach / peak, "traffic": traffic, "bytes_per_update": BYTES_PER_UPDATE,
+                     "frac": ach / peak, "traffic": traffic, "traffic_build": NCU_TRAFFIC_BYTES.get(cfg.name, {}).get("build"),
+                     "bytes_per_update": BYTES_PER_UPDATE,
                      "algorithmic_bytes_per_launch": per_launch_bytes[dom],
                      # the second denominator SURVEY.md 8(d) asks for, labelled: ncu's theoretical DRAM peak, and the
                      # dram throughput % ncu itself reported for this kernel in the committed capture (profiles/)
@@ -284,6 +322,9 @@ def run_ours(args, cfg):
         "clocks": clocks,
         "observables_rank0": {"E_per_site": obs[0, 0] / N, "m": float(np.sqrt(obs[0, 3])) / N},
     }
+    if world == 1 and not args.no_other_workloads and not any((args.tile_y, args.tile_z, args.generic_kernel, args.slot_chunk)):
+        xy.close()
+        out["other_workloads"] = time_other_workloads(binding, torch, cfg.name)
     if not args.no_cpu_baseline and world == 1:
         cores = os.cpu_count() or 1
         n_slots = max(1, min(R, cores))
@@ -306,6 +347,7 @@ def main():
                                                   "non-uniform (geometric) ladder; see inputs.PAPER_FAMILIES")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-workloads", action="store_true", help="skip the short timings of the other configs / paper families")
     ap.add_argument("--tile-z", type=int, default=0, help="override the march length (tuning; 0 = library default)")
     ap.add_argument("--tile-y", type=int, default=0, help="override the tile rows (tuning; 0 = library default)")
     ap.add_argument("--generic-kernel", action="store_true", help="force the run-time-geometry colour-pass kernel (tuning)")
