@@ -173,7 +173,7 @@ void default_tiles_z(int L, int R, int TY, int& TZ) {
 
 bool tiles_ok(int L, int TY, int TZ) {
     return TY >= 2 && TZ >= 2 && L % TY == 0 && L % TZ == 0 && TY * (L / 8) <= 352 &&   // 11 compute warps + the auxiliary warp
-           sweep_smem_bytes(L, TY) <= 200 * 1024;
+           sweep_smem_bytes_max(L, TY) <= 200 * 1024;
 }
 
 template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE, int W4C, int TYC>
@@ -185,7 +185,7 @@ int launch_sweep_impl(xy_ctx* c, const SweepParams& P) {
         CK(cudaFuncSetAttribute(sweep_kernel<MODE, TRACE, FUSED, EXACT_INLINE, W4C, TYC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_set[c->device].store(true, std::memory_order_release);
     }
-    const size_t smem = sweep_smem_bytes(P.L, P.TY);
+    const size_t smem = sweep_smem_bytes(P.L, P.TY, W4C != 0 && (W4C * TYC / 2) % 32 == 0);   // the kernel's UNI mapping
     const int threads = (P.nItems + 31) / 32 * 32 + 32;          // compute warps + the auxiliary warp
     dim3 grid(P.nTY * P.nTZ, P.n_slots);
     {

@@ -123,10 +123,33 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
 }
 
 
-// Shared memory of one block (bytes):  kRing staged planes of (TY+2) rows x W pairs x 8  |
+// Padding of a staged row (bytes, a multiple of 16).  A warp's 128-bit accesses to a staged row go to consecutive
+// 16-byte words, eight lanes per wavefront; where a warp continues in its NEXT row (the row `jump` staged rows further:
+// 1 in the row-major thread mapping, 2 where the warps are mapped to rows of one parity), the eight lanes around the
+// break still hit eight different bank groups only if that row starts where this one's part ended, modulo the 128
+// bytes of the banks:  jump * (W4*32 + pad) == W4*16  (mod 128).  Without padding this fails whenever W4 is not a
+// multiple of 8 (L = 160: W4 = 20, 3.3e6 + 1.9e6 excess wavefronts per launch on the loads of the rows above / below
+// and on the staging stores; profiles/r3_head.md).  0 where no multiple of 16 solves it or XY_STAGE_PAD is 0.
+#ifndef XY_STAGE_PAD
+#define XY_STAGE_PAD 1
+#endif
+__host__ __device__ constexpr int stage_pad_bytes(int W4, bool uni) {
+    if (!XY_STAGE_PAD) return 0;
+    for (int pad = 0; pad < 128; pad += 16)
+        if (((uni ? 2 : 1) * (W4 * 32 + pad) - W4 * 16) % 128 == 0) return pad;
+    return 0;
+}
+
+// Shared memory of one block (bytes):  kRing staged planes of (TY+2) rows x (W pairs x 8 + padding)  |
 // kRaw raw slots of (2 TY + 2) rows x W floats x 4 (other colour first, then own)  |  1 + kRaw mbarriers
-__host__ __device__ inline size_t sweep_smem_bytes(int L, int TY) {
-    return (size_t)kRing * (TY + 2) * (L / 2) * 8 + (size_t)kRaw * (2 * TY + 2) * (L / 2) * 4 + 8 * (1 + kRaw) + 8;
+// uni: the warps of the kernel variant are mapped to rows of one parity (compile-time geometry, see sweep_kernel)
+__host__ __device__ inline size_t sweep_smem_bytes(int L, int TY, bool uni = false) {
+    return (size_t)kRing * (TY + 2) * ((L / 2) * 8 + stage_pad_bytes(L / 8, uni)) + (size_t)kRaw * (2 * TY + 2) * (L / 2) * 4 + 8 * (1 + kRaw) + 8;
+}
+// the larger of the two mappings' needs (tile validation on the host, before a kernel variant is chosen)
+__host__ __device__ inline size_t sweep_smem_bytes_max(int L, int TY) {
+    const size_t a = sweep_smem_bytes(L, TY, false), b = sweep_smem_bytes(L, TY, true);
+    return a > b ? a : b;
 }
 
 // W4C, TYC: L/8 and the tile rows as compile-time constants (every shared-memory pitch becomes an
@@ -150,7 +173,7 @@ __global__ void __launch_bounds__(W4C ? (W4C * TYC + 31) / 32 * 32 + 32 : 384, (
     const int W4 = W4C ? W4C : P.W4;
     const int W = 4 * W4;
     const int TY = TYC ? TYC : P.TY, TZ = P.TZ;
-    const int rowB = W * 8;                          // bytes per staged row (W pairs)
+    const int rowB = W * 8 + stage_pad_bytes(W4, UNI);   // bytes per staged row (W pairs + bank padding)
     const int partB = W4 * 16;                       // byte offset of part B inside a row
     const int planeB = (TY + 2) * rowB;              // bytes per staged plane; ring of kRing planes
     const int ringB = kRing * planeB;
