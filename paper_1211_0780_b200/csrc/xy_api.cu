@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstring>
 #include <mutex>
+#include <utility>
 #include <vector>
 
 #include "xy_kernels.cuh"
@@ -90,6 +91,7 @@ struct xy_ctx {
     uint32_t n_met = 0, n_or = 0, n_pt = 0;
     // device
     int device = -1;                           // the CUDA device of the attached buffers and stream (xy_attach)
+    int sm_count = 148;                        // its multiprocessors (xy_attach)
     bool attached = false;
     float* d_state = nullptr; bool own_state = false;
     char* d_ws = nullptr; bool own_ws = false;
@@ -176,23 +178,51 @@ bool tiles_ok(int L, int TY, int TZ) {
            sweep_smem_bytes_max(L, TY) <= 200 * 1024;
 }
 
+// Launches one kernel of the step's chain.  With XY_PDL the launch carries the programmatic-stream-serialization
+// attribute (xy_device.cuh): its blocks may become resident during the tail of the previous kernel on the stream and
+// wait there (grid_dependency_wait) until that kernel has completed.  Profiling puts event records between the
+// launches, which serialises them the ordinary way.
+template <class... KArgs, class... Args>
+cudaError_t launch_chained(bool pdl, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args&&... args) {
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
+// Where it pays: the saving is a few microseconds per kernel boundary, so +1 ... +5 % per step for passes of up to ~7
+// blocks per multiprocessor (L = 64 ... 128 x 34 replicas, L = 160 x 13; profiles/r3_experiments.md), while at
+// L = 160 x 64 (9-11 blocks per multiprocessor and pass) the step was 0.15 % SLOWER with it, repeatably.  Hence the bound.
+bool chain_pdl(const xy_ctx* c) {
+    return XY_PDL != 0 && (long)c->R * (c->L / c->TY) * (c->L / c->TZ) <= 8L * c->sm_count;
+}
+
 template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE, int W4C, int TYC>
 int launch_sweep_impl(xy_ctx* c, const SweepParams& P) {
-    // The dynamic-shared-memory opt-in is a per-device attribute of each instantiation: one flag per device,
-    // set outside any stream capture (xy_mcs launches its first step eagerly).
+    // Two instantiations per variant: with and without the grid-dependency instructions (the test hook and the
+    // large-|beta| variant only without).  The dynamic-shared-memory opt-in is a per-device attribute of each: one flag
+    // per device, set outside any stream capture (xy_mcs launches its first step eagerly).
+    constexpr bool CAN_PDL = XY_PDL != 0 && !TRACE && !EXACT_INLINE;
+    auto plain = sweep_kernel<MODE, TRACE, FUSED, EXACT_INLINE, W4C, TYC, false>;
+    auto chained = sweep_kernel<MODE, TRACE, FUSED, EXACT_INLINE, W4C, TYC, CAN_PDL>;
     static std::atomic<bool> attr_set[kMaxDevices];
     if (!attr_set[c->device].load(std::memory_order_acquire)) {
-        CK(cudaFuncSetAttribute(sweep_kernel<MODE, TRACE, FUSED, EXACT_INLINE, W4C, TYC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        CK(cudaFuncSetAttribute(plain, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        if (CAN_PDL) CK(cudaFuncSetAttribute(chained, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_set[c->device].store(true, std::memory_order_release);
     }
     const size_t smem = sweep_smem_bytes(P.L, P.TY, W4C != 0 && (W4C * TYC / 2) % 32 == 0);   // the kernel's UNI mapping
     const int threads = (P.nItems + 31) / 32 * 32 + 32;          // compute warps + the auxiliary warp
     dim3 grid(P.nTY * P.nTZ, P.n_slots);
+    const bool pdl = CAN_PDL && chain_pdl(c);
     {
         LaunchSpan span(c, MODE == MODE_MET ? XY_K_METROPOLIS : MODE == MODE_OR ? XY_K_OVERRELAX : XY_K_MEASURE);   // MODE_STIFF counts as measure
-        sweep_kernel<MODE, TRACE, FUSED, EXACT_INLINE, W4C, TYC><<<grid, threads, smem, c->stream>>>(P);
+        CK(launch_chained(pdl, pdl ? chained : plain, grid, dim3(threads), smem, c->stream, P));
     }
-    CK(cudaGetLastError());
     return XY_OK;
 }
 
@@ -539,6 +569,7 @@ int xy_attach(xy_ctx* c, void* d_state, void* d_workspace, void* cuda_stream) {
     CK(cudaGetDeviceProperties(&prop, dev));
     if (dev < 0 || dev >= kMaxDevices) return fail(XY_ERR_NO_DEVICE, "xy_attach: device index %d out of range", dev);
     c->device = dev;
+    c->sm_count = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : 148;
     if (prop.major < 10) return fail(XY_ERR_NO_DEVICE, "xy_attach: device %s is sm_%d%d; built for sm_100a only", prop.name, prop.major, prop.minor);
     if (((uintptr_t)d_state | (uintptr_t)d_workspace) & 255u) return fail(XY_ERR_INVALID_ARG, "xy_attach: buffers must be 256-byte aligned");
     for (void* p : { d_state, d_workspace }) {        // caller-owned buffers must live on the device this context is bound to
@@ -667,9 +698,8 @@ static int metropolis_slots(xy_ctx* c, int slot0, int n_slots) {
             F.done_ticket = P.near_count + 1; F.overflow_flag = P.near_count + 2;
             {
                 LaunchSpan span(c, XY_K_FIXUP);
-                met_fixup_kernel<<<148, 256, 0, c->stream>>>(F);
+                CK(launch_chained(chain_pdl(c), met_fixup_kernel, dim3(148), dim3(256), 0, c->stream, F));
             }
-            CK(cudaGetLastError());
         }
     }
     return XY_OK;
@@ -732,12 +762,12 @@ static int pt_exchange_impl(xy_ctx* c, double* d_series_row) {
     if (!from_slots && (!c->rank_valid || d_series_row || c->device_counters)) {
         const int n_tiles = (c->L / c->TY) * (c->L / c->TZ);
         LaunchSpan span(c, XY_K_PT);
-        finalize_pt_kernel<<<1, 1024, 0, c->stream>>>(
-            c->ws_ptr<double>(c->ws.partials), n_tiles, c->R, c->n_pt, c->keys, c->ws_ptr<double>(c->ws.betas),
+        CK(launch_chained(chain_pdl(c), finalize_pt_kernel, dim3(1), dim3(1024), 0, c->stream,
+            (const double*)c->ws_ptr<double>(c->ws.partials), n_tiles, c->R, c->n_pt, c->keys, (const double*)c->ws_ptr<double>(c->ws.betas),
             c->ws_ptr<int>(c->ws.slot_at_rank), c->ws_ptr<double>(c->ws.obs_rank), c->ws_ptr<double>(c->ws.obs_slot),
             d_series_row, c->ws_ptr<double>(c->ws.beta_of_slot), c->ws_ptr<float>(c->ws.beta32),
             c->ws_ptr<unsigned long long>(c->ws.pt_acc),
-            c->device_counters ? c->ws_ptr<DeviceCounters>(c->ws.dctr) : nullptr, c->or_per_mcs);
+            c->device_counters ? c->ws_ptr<DeviceCounters>(c->ws.dctr) : (DeviceCounters*)nullptr, c->or_per_mcs));
     } else {
         const int pairs = c->R / 2 + 1;
         LaunchSpan span(c, XY_K_PT);

@@ -8,6 +8,31 @@
 namespace xyk {
 
 // ---------------------------------------------------------------------------------------------
+// Programmatic dependent launch.  The kernels of one Monte Carlo step form a chain on one stream (Metropolis pass,
+// settlement, Metropolis pass, settlement, two over-relaxation passes, final reduction + exchange).  Launched with
+// cudaLaunchAttributeProgrammaticStreamSerialization, a kernel's blocks may become resident while the tail of its
+// predecessor still runs: they do their prologue (mbarrier set-up), then grid_dependency_wait() holds them until the
+// predecessor has COMPLETED and its writes are visible -- so the data dependences are exactly those of a plain
+// stream, only the launch latency and the prologue move off the critical path.  allow_dependent_launch() lets the
+// successor's blocks take the multiprocessors this grid no longer fills once every block of this grid has started.
+// Every kernel of the chain calls both before its first access to global memory; without the launch attribute
+// both are no-ops.  XY_PDL = 0 compiles them out.
+// ---------------------------------------------------------------------------------------------
+#ifndef XY_PDL
+#define XY_PDL 1
+#endif
+__device__ __forceinline__ void allow_dependent_launch() {
+#if XY_PDL
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+#endif
+}
+__device__ __forceinline__ void grid_dependency_wait() {
+#if XY_PDL
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
+}
+
+// ---------------------------------------------------------------------------------------------
 // Philox4x32-10 (Salmon et al., SC'11) -- north_star "generated in registers"; replaces the
 // Warp Generator of P:30.  The ten round keys depend only on the seed, so the host computes
 // them once and the kernels read them from the constant bank (no per-thread key schedule).

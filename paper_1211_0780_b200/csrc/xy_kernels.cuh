@@ -36,6 +36,8 @@ struct FixupParams {
 };
 
 __global__ void __launch_bounds__(256) met_fixup_kernel(const FixupParams F) {
+    allow_dependent_launch();
+    grid_dependency_wait();                      // the colour pass that filled the queue has completed
     const unsigned int n_raw = *F.near_count;
     const unsigned int n = n_raw < F.near_cap ? n_raw : F.near_cap;
     const int L = F.L, W = F.W;
@@ -181,6 +183,8 @@ __global__ void __launch_bounds__(1024) finalize_pt_kernel(const double* __restr
                                                           double* __restrict__ beta_of_slot, float* __restrict__ beta32_of_slot,
                                                           unsigned long long* __restrict__ pt_acc, DeviceCounters* __restrict__ dc,
                                                           int or_per_mcs) {
+    allow_dependent_launch();
+    grid_dependency_wait();                      // the pass that wrote the partial sums has completed
     if (dc) {                                    // CUDA-graph replay: this step's counters live on the device
         n_pt = dc->n_pt;
         series_row = dc->series_base ? dc->series_base + (size_t)dc->row * R * 5 : nullptr;

@@ -165,7 +165,7 @@ __host__ __device__ inline size_t sweep_smem_bytes_max(int L, int TY) {
 #ifndef XY_MET_EARLY_DRAW
 #define XY_MET_EARLY_DRAW 1
 #endif
-template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE, int W4C, int TYC>
+template <int MODE, bool TRACE, bool FUSED, bool EXACT_INLINE, int W4C, int TYC, bool PDL = false>
 __global__ void __launch_bounds__(W4C ? (W4C * TYC + 31) / 32 * 32 + 32 : 384, (W4C * TYC > 352) ? 1 : XY_SWEEP_MIN_BLOCKS) sweep_kernel(const SweepParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr bool UNI = W4C != 0 && (W4C * TYC / 2) % 32 == 0;   // whole warps per row parity (L = 80: compile-time geometry only)
@@ -203,6 +203,14 @@ __global__ void __launch_bounds__(W4C ? (W4C * TYC + 31) / 32 * 32 + 32 : 384, (
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
+    // everything above touched shared memory only; from here on the kernel reads what its predecessor wrote
+    // PDL: this instantiation is launched with programmatic stream serialization (xy_device.cuh).  A template parameter,
+    // not a run-time flag: the mere presence of the two instructions cost the over-relaxation pass 0.2-0.3 % at
+    // L = 160 x 64, where the launcher does not use them (profiles/r3_experiments.md)
+    if (PDL) {
+        allow_dependent_launch();
+        grid_dependency_wait();
+    }
 
     constexpr bool MEAS = (MODE == MODE_MEASURE) || FUSED;
     constexpr bool STIFF = MODE == MODE_STIFF;          // the six bond sums of Eq. 6 instead of E, Mx, My
