@@ -146,20 +146,35 @@ struct LaunchSpan {
     }
 };
 
-void default_tiles_z(int L, int R, int TY, int& TZ);
+// Multiprocessors of the device the tiles are chosen for: the current device if there is one (a query only -- no
+// context is created, nothing is allocated), else a full B200.  The tile models below count block slots in units of
+// this number instead of assuming 148.
+constexpr int kB200Sms = 148;
+int current_sm_count() {
+    int n_dev = 0, dev = 0, sms = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) { cudaGetLastError(); return kB200Sms; }
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
+        cudaGetLastError();
+        return kB200Sms;
+    }
+    return sms;
+}
 
-void default_tiles(int L, int R, int& TY, int& TZ) {
+void default_tiles_z(int L, int R, int TY, int& TZ, int sms);
+
+void default_tiles(int L, int R, int& TY, int& TZ, int sms = 0) {
+    if (sms <= 0) sms = current_sm_count();
     const int W4 = L / 8;
     TY = 2;                                        // L up to 1024: TY * L/8 must stay within 11 compute warps
     for (int t = 2; t <= L; ++t)
         if (L % t == 0 && t * W4 <= 320) TY = t;
-    default_tiles_z(L, R, TY, TZ);
+    default_tiles_z(L, R, TY, TZ, sms);
 }
 
-// March length for tile rows TY.
-void default_tiles_z(int L, int R, int TY, int& TZ) {
+// March length for tile rows TY on a device of `sms` multiprocessors.
+void default_tiles_z(int L, int R, int TY, int& TZ, int sms) {
     // A block costs TZ + 2 steps (two of them only stage) plus the latency of its first copies (about
-    // 1.5 step-times), and 2 blocks fit an SM.  With w = blocks / (2 * 148 SMs) "waves" the pass takes about
+    // 1.5 step-times), and 2 blocks fit an SM.  With w = blocks / (2 * sms) "waves" the pass takes about
     // (max(w, 1/2) + 0.3) * (TZ + 3.5) step-times: blocks end at different times, so a fraction of a wave is lost at the
     // end, not a whole one, and an SM that holds one block instead of two runs it faster.  Take the divisor of L that
     // minimises it.  Fitted to the measured march-length sweeps at L = 64, 128, 160 (profiles/r2_experiments.md).
@@ -167,7 +182,7 @@ void default_tiles_z(int L, int R, int TY, int& TZ) {
     double best = 1e300;
     for (int t = L; t >= 2; --t) {
         if (L % t) continue;
-        const double w = (double)((long)R * (L / TY) * (L / t)) / 296.0;
+        const double w = (double)((long)R * (L / TY) * (L / t)) / (2.0 * sms);
         const double cost = (std::fmax(w, 0.5) + 0.3) * (t + 3.5);
         if (cost < best * 0.999) { best = cost; TZ = t; }
     }
@@ -334,7 +349,7 @@ int check_near_overflow(xy_ctx* c) {
 
 int grid_for(size_t n_items, int threads) {
     size_t b = (n_items + threads - 1) / threads;
-    const size_t cap = 148 * 16;
+    static const size_t cap = (size_t)current_sm_count() * 16;      // grid-stride kernels: 16 blocks per multiprocessor at most
     return (int)(b < 1 ? 1 : (b > cap ? cap : b));
 }
 
@@ -508,7 +523,9 @@ xy_ctx* xy_create(int L, int R, const double* betas, uint64_t seed) {
     c->betas.assign(betas, betas + R);
     c->keys = philox_round_keys((uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32));
     c->ws = ws_layout(L, R);
-    default_tiles(L, R, c->TY, c->TZ);
+    const int sms = current_sm_count();
+    c->sm_count = sms;                             // xy_attach replaces it by the bound device's
+    default_tiles(L, R, c->TY, c->TZ, sms);
     if (!tiles_ok(L, c->TY, c->TZ)) {
         fail(XY_ERR_INVALID_ARG, "xy_create: no valid tile for L=%d (TY=%d TZ=%d)", L, c->TY, c->TZ);
         delete c;
@@ -522,7 +539,7 @@ xy_ctx* xy_create(int L, int R, const double* betas, uint64_t seed) {
         for (int t = L; t >= 2; --t) {
             if (L % t) continue;
             const long blocks = (long)R * (L / c->TY_met) * (L / t);
-            const double cost = (double)((blocks + 147) / 148) * (t + 1.0);
+            const double cost = (double)((blocks + sms - 1) / sms) * (t + 1.0);
             if (cost < best * 0.999) { best = cost; c->TZ_met = t; }
         }
     }
@@ -530,7 +547,7 @@ xy_ctx* xy_create(int L, int R, const double* betas, uint64_t seed) {
     // (L = 96 with warps of uniform x parity; L = 80: 0.1587 -> 0.1526 ms per step at R = 34 against 20 rows, run-time geometry)
     if ((L == 96 || L == 80) && tiles_ok(L, 16, c->TZ)) {
         c->TY = 16;
-        default_tiles_z(L, R, 16, c->TZ);
+        default_tiles_z(L, R, 16, c->TZ, sms);
         // measured at the paper's R = 34 (bench.py --family): L = 80: TZ 16 0.1468 ms per step against 0.1526 (20), 0.1786 (40);
         // L = 96: TZ 24 0.2405 against 0.2594 (32) -- three blocks of these small tiles fit an SM, which the model does not know
         if (R >= 24 && R <= 48) c->TZ = L == 80 ? 16 : 24;
@@ -698,7 +715,7 @@ static int metropolis_slots(xy_ctx* c, int slot0, int n_slots) {
             F.done_ticket = P.near_count + 1; F.overflow_flag = P.near_count + 2;
             {
                 LaunchSpan span(c, XY_K_FIXUP);
-                CK(launch_chained(chain_pdl(c), met_fixup_kernel, dim3(148), dim3(256), 0, c->stream, F));
+                CK(launch_chained(chain_pdl(c), met_fixup_kernel, dim3(c->sm_count), dim3(256), 0, c->stream, F));
             }
         }
     }
