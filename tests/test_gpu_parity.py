@@ -885,6 +885,36 @@ def test_free_run_is_reproducible_across_kernel_variants(xy_mod, L, R):
         assert np.allclose(obs[:, :3], ref[2][:, :3], rtol=0, atol=1e-6 * 3 * L ** 3), v
 
 
+@pytest.mark.parametrize("L,R", [(64, 3), (96, 2), (160, 1)])
+def test_chained_launches_equal_serialised_launches(xy_mod, L, R):
+    """Programmatic dependent launch (the kernels of a step may become resident during their predecessor's tail and
+    wait there for its completion) must not change a single bit.  XY_OPT_PROFILE = 1 puts an event record between any
+    two launches, which is plain stream order without overlap, and disables graph replay: 8 steps that way against 8
+    steps the default way (first step eager, then the captured graph with programmatic edges), and against 8 single
+    sweep-by-sweep calls."""
+    betas = inputs.beta_ladder(0.4535, 0.4550, R)
+    runs = []
+    for mode in ("default", "profiled", "stepwise"):
+        xy = xy_mod.XY(L, R, betas, SEED)
+        xy.set_option(xy_mod.XY_OPT_RESIDENT, 0)
+        xy.set_option(xy_mod.XY_OPT_PROFILE, 1 if mode == "profiled" else 0)
+        xy.init_random()
+        if mode == "stepwise":
+            for _ in range(8):
+                xy.metropolis_sweep(); xy.overrelax_sweep(); xy.measure(to_host=False); xy.pt_exchange()
+        else:
+            xy.mcs(8)
+        runs.append((xy.get_state(), xy.get_perm(), xy.get_accept_counts(), xy.measure()))
+        if mode == "profiled":
+            kt = xy.get_kernel_times()
+            assert kt["metropolis"][1] == 16 and kt["overrelax"][1] == 16 and kt["fixup"][1] == 16, kt
+    for other in runs[1:]:
+        assert np.array_equal(runs[0][0].view(np.uint32), other[0].view(np.uint32))
+        assert np.array_equal(runs[0][1], other[1])
+        assert np.array_equal(runs[0][2][0], other[2][0]) and np.array_equal(runs[0][2][1], other[2][1])
+        assert np.array_equal(runs[0][3], other[3])
+
+
 @pytest.mark.parametrize("L,R,chunk,n_or", [(32, 5, 2, 1), (64, 3, 1, 2), (160, 3, 2, 1)])
 def test_slot_chunk_schedule_equals_default(xy_mod, L, R, chunk, n_or):
     """XY_OPT_SLOT_CHUNK (SURVEY 8(f) f2 for large lattices: the four colour passes of K slots back to back, so that
